@@ -1,0 +1,141 @@
+/* mgrhd.h -- C ABI of the B200-native per-cell implicit matter-radiation source update
+ * of arXiv 2407.18304 (He, Wibking & Krumholz), Section 3, PAPER.md:373-467 (Eq. 37-52),
+ * with the group-mean opacities of Section 2.2 (Eq. 17-31).
+ *
+ * One call of mgrhd_source_update() advances every cell of a structure-of-arrays state from
+ * the post-explicit state U^(t) to U^(t+1) by solving Eq. 37-40 with the paper's inner Newton
+ * iteration on x = (E_gas, R_1..R_Nq) (Eq. 41-50; arrowhead Jacobian of Eq. 48 eliminated in
+ * O(Nq)) and outer iteration on the lagged (v, F_g) (Eq. 51-52).
+ *
+ * All arithmetic is IEEE double precision on the device.  There is no CPU fallback: every
+ * entry point that computes returns MGRHD_ERR_CUDA when no CUDA device can be used.
+ *
+ * Conventions (energy-density units; 4*pi/c never appears):
+ *   x = h nu/(k_B T);  Bt_g = 4 pi B_g/c = a_R T^4 [Y(x_g+) - Y(x_g-)],
+ *   Y(x) = (15/pi^4) int_0^x t^3/(e^t-1) dt  (Eq. 11 applied to the Planck function).
+ *   chi_{0,g-} = rho * kappa_scale * kappa_lo[g] (absorption coefficient, 1/length), Eq. 19.
+ *   C_v = rho k_B/((gamma-1) mean_mass) (volumetric), T = (E_gas - |rho v|^2/(2 rho))/C_v.
+ *   Conserved by construction: E_gas + (c/c_hat) sum_g E_g and
+ *   rho v + (c c_hat)^-1 sum_g F_g.
+ */
+#ifndef MGRHD_H
+#define MGRHD_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define MGRHD_MAX_GROUPS 64   /* largest Nq accepted (BASELINE.json config 5) */
+#define MGRHD_HIST 64         /* iteration histograms are clamped to this many bins */
+
+enum {
+  MGRHD_OK = 0,
+  MGRHD_ERR_ARG = -1,        /* null pointer, Nq out of range, ncells < 0, bad enum value      */
+  MGRHD_ERR_RANGE = -2,      /* dt <= 0, c <= 0, c_hat <= 0 or c_hat > c, non-positive units    */
+  MGRHD_ERR_EDGES = -3,      /* edges not strictly ascending, negative, or NaN                  */
+  MGRHD_ERR_ALPHA = -4,      /* alpha != 0 in a group whose edge is 0 or +inf (Eq. 19 undefined) */
+  MGRHD_ERR_CUDA = -5        /* CUDA runtime failure; mgrhd_last_error() has the text           */
+};
+
+typedef struct mgrhd_ctx mgrhd_ctx; /* opaque; created by mgrhd_init, destroyed by mgrhd_free */
+
+/* Physical constants in the caller's unit system (independent inputs). */
+typedef struct {
+  double a_rad;      /* radiation constant a_R                       */
+  double k_B;        /* Boltzmann constant                           */
+  double h_planck;   /* Planck constant                              */
+  double mean_mass;  /* mean particle mass mu*m_H                    */
+  double gamma;      /* adiabatic index; C_v = rho k_B/((gamma-1) mean_mass) */
+} mgrhd_units;
+
+/* Opacity model and iteration controls.  HOST pointers, copied by mgrhd_init. */
+typedef struct {
+  const double *kappa_lo;  /* [Nq] specific opacity at each group's LOWER edge (Eq. 19)        */
+  const double *alpha;     /* [Nq] in-group power-law slope alpha_{chi0,g}; 0 => PC (Eq. 17)   */
+  int closure;             /* 0 = Levermore/M1, 1 = Eddington P = E/3 I (:603)  */
+  int spectrum;            /* 0 = PPL fixed slope alpha_Q = -1; others rejected */
+  double newton_tol;       /* epsilon of Eq. 49 (paper default 1e-11)            */
+  int newton_maxit;        /* cap on Newton steps per outer trip (paper silent; 50)            */
+  int outer_maxit;         /* cap on outer trips (paper silent; 50)                            */
+  double outer_tol;        /* 1e-13 of PAPER.md:465                                            */
+  int outer_stop;          /* 0 = paper rule only; 1 = also |dF_g|<=rel*|F_g|, |d rho v|<=rel*|rho v| */
+  double outer_rel_tol;    /* rel of outer_stop == 1 (1e-12)                                   */
+} mgrhd_opacity_model;
+
+/* Cell state, structure of arrays, float64, cell index fastest.  In mgrhd_source_update all
+ * pointers are DEVICE pointers owned by the caller; mom, Egas, Erad, Frad are updated in
+ * place, rho and kappa_scale are read only.  Arrays must not alias one another. */
+typedef struct {
+  const double *rho;         /* [n]      gas density                                           */
+  double *mom[3];            /* [n] each rho v                                                 */
+  double *Egas;              /* [n]      gas TOTAL energy density (internal + kinetic), Eq. 12 */
+  double *Erad;              /* [Nq][n]  group radiation energy density E_g                    */
+  double *Frad[3];           /* [Nq][n]  each: group radiation flux F_g^i                      */
+  const double *kappa_scale; /* [n] per-cell multiplier on kappa_lo, or NULL (= 1)             */
+} mgrhd_state;
+
+/* Per-call diagnostics, accumulated on the device since the last mgrhd_reset_stats(). */
+typedef struct {
+  long long n_cells;                   /* cells processed                                       */
+  long long n_newton_unconverged;      /* inner loops that hit newton_maxit                     */
+  long long n_outer_unconverged;       /* cells that hit outer_maxit                            */
+  long long n_T_nonpositive_steps;     /* Newton steps halved to keep T > 0, + invalid inputs   */
+  long long n_chiF_guard;              /* cell-groups whose Eq. 27 denominator underflowed      */
+  long long n_denominator_nonpositive; /* cell-groups with 1 + c_hat chi_F dt <= 0              */
+  long long newton_evals_total;        /* residual evaluations (Eq. 41), summed over cells      */
+  long long outer_trips_total;         /* outer trips, summed over cells                        */
+  long long newton_hist[MGRHD_HIST];   /* per-cell residual evaluations (clamped)               */
+  long long outer_hist[MGRHD_HIST];    /* per-cell outer trips (clamped)                        */
+} mgrhd_stats;
+
+/* Create a context for one group structure / unit system / opacity model.
+ *   group_edges [Nq+1] HOST: nu_{g-}, ascending, >= 0; the last may be +inf.
+ *   1 <= Nq <= MGRHD_MAX_GROUPS.  The context copies everything it needs (tables go to
+ *   constant memory at launch); it uses the CUDA device current at the time of the call.
+ * Returns MGRHD_OK and *out, or a negative error (and *out = NULL). */
+int mgrhd_init(mgrhd_ctx **out, const double *group_edges, int Nq,
+               const mgrhd_units *units, const mgrhd_opacity_model *model);
+
+/* One implicit source update (Eq. 37-52) of `ncells` cells, in place, with dt = theta*Delta t
+ * (PAPER.md:389), speed of light c and reduced speed of light c_hat <= c (Eq. 34).
+ * Stream-ordered on `cuda_stream` (a cudaStream_t, NULL = default stream), asynchronous:
+ * no host synchronisation, no allocation.  ncells == 0 is a no-op.  Per-cell numerical
+ * failures never abort; they are counted in mgrhd_stats. */
+int mgrhd_source_update(mgrhd_ctx *ctx, const mgrhd_state *state_dev, long long ncells,
+                        double dt, double c, double c_hat, void *cuda_stream);
+
+/* The same update for a state held in HOST memory (pinned or pageable): the cells are cut
+ * into slabs that are copied to the device, updated and copied back on alternating streams,
+ * so copies overlap kernels.  Synchronous: returns when the host arrays hold U^(t+1).
+ * Scratch device memory (a few hundred MB) is owned by the context and reused. */
+int mgrhd_source_update_host(mgrhd_ctx *ctx, const mgrhd_state *state_host, long long ncells,
+                             double dt, double c, double c_hat);
+
+/* Per-cell conserved totals of a DEVICE state, for conservation checks:
+ *   out_energy[n]      = E_gas + (c/c_hat) sum_g E_g
+ *   out_momentum[3][n] = rho v^i + (c c_hat)^-1 sum_g F_g^i
+ * Stream-ordered, asynchronous. */
+int mgrhd_conserved_totals(mgrhd_ctx *ctx, const mgrhd_state *state_dev, long long ncells,
+                           double c, double c_hat, double *out_energy, double *out_momentum,
+                           void *cuda_stream);
+
+/* Copy the device counters to *host_out (synchronises the last stream used). */
+int mgrhd_get_stats(mgrhd_ctx *ctx, mgrhd_stats *host_out);
+/* Zero the device counters (stream-ordered on the last stream used). */
+int mgrhd_reset_stats(mgrhd_ctx *ctx);
+/* Number of kernels this context has launched so far (for bench.py's gpu_launches). */
+long long mgrhd_launch_count(const mgrhd_ctx *ctx);
+
+/* Sustained FP64 FMA rate of the current device in FMA/s (a dependent-chain-free DFMA
+ * microbenchmark, `iters` FMAs per thread; used as the ALU roofline denominator). */
+int mgrhd_measure_dfma_peak(long long iters, double *fma_per_second);
+
+/* Text of the last CUDA error seen by this library on the calling thread ("" if none). */
+const char *mgrhd_last_error(void);
+
+void mgrhd_free(mgrhd_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MGRHD_H */

@@ -1,0 +1,347 @@
+// mgrhd_api.cu -- host side of the C ABI declared in include/mgrhd.h: argument checks,
+// table generation, launches, the slab-pipelined host-buffer path and diagnostics.
+// Product code; shares nothing with oracle/.  No CPU fallback anywhere: every computing
+// entry point launches the CUDA kernels of mgrhd_kernels.cuh or fails.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <mutex>
+#include <new>
+
+#include "mgrhd_kernels.cuh"
+
+using namespace mgrhd;
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+bool cuda_ok(cudaError_t e, const char* what) {
+  if (e == cudaSuccess) return true;
+  std::snprintf(g_err, sizeof g_err, "%s: %s", what, cudaGetErrorString(e));
+  return false;
+}
+#define CU(call) do { if (!cuda_ok((call), #call)) return MGRHD_ERR_CUDA; } while (0)
+
+// zeta(2n) for n >= 1 in long double: direct sum + Euler-Maclaurin tail.
+long double zeta_even(int n) {
+  const long double PI = 3.14159265358979323846264338327950288L;
+  if (n == 1) return PI * PI / 6.0L;
+  if (n == 2) return PI * PI * PI * PI / 90.0L;
+  const int s = 2 * n, M = 64;
+  long double sum = 0.0L;
+  for (int k = M - 1; k >= 1; --k) sum += powl((long double)k, -(long double)s);
+  const long double m = (long double)M;
+  // tail: int_M^inf x^-s dx + M^-s/2 + s M^(-s-1)/12 - s(s+1)(s+2) M^(-s-3)/720
+  sum += powl(m, 1.0L - s) / (s - 1.0L) + 0.5L * powl(m, -(long double)s) +
+         s * powl(m, -s - 1.0L) / 12.0L - s * (s + 1.0L) * (s + 2.0L) * powl(m, -s - 3.0L) / 720.0L;
+  return sum;
+}
+
+// b_{2n} = B_{2n}/(2n)! = (-1)^(n+1) 2 zeta(2n)/(2 pi)^(2n): Maclaurin coefficients of
+// t/(e^t-1) = 1 - t/2 + sum_n b_{2n} t^(2n).
+void fill_planck_tables(PlanckTables& t) {
+  const long double TWO_PI = 6.28318530717958647692528676655900577L;
+  for (int n = 1; n <= kSmallTerms; ++n) {
+    long double b = 2.0L * zeta_even(n) / powl(TWO_PI, 2.0L * n);
+    if (n % 2 == 0) b = -b;
+    t.xi_c[n - 1] = (double)b;
+    t.y_c[n - 1] = (double)(b / (2.0L * n + 3.0L));
+  }
+  t.inv_n[0] = 0.0;
+  for (int n = 1; n <= kSeriesMax; ++n) t.inv_n[n] = (double)(1.0L / (long double)n);
+}
+
+std::once_flag g_tables_once[16];  // per device
+cudaError_t g_tables_err[16];
+
+cudaError_t upload_tables_for_current_device() {
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= 16) return cudaErrorInvalidDevice;
+  std::call_once(g_tables_once[dev], [dev]() {
+    PlanckTables t;
+    fill_planck_tables(t);
+    g_tables_err[dev] = cudaMemcpyToSymbol(c_planck, &t, sizeof t);
+  });
+  return g_tables_err[dev];
+}
+
+constexpr int kBlock = 128;
+constexpr int kSlabs = 3;                       // host path: slabs in flight
+constexpr long long kSlabBytes = 96ll << 20;    // target bytes per slab
+
+}  // namespace
+
+struct mgrhd_ctx {
+  Params P;
+  int device;
+  int sm_count;
+  unsigned long long* d_stats;
+  cudaStream_t last_stream;
+  long long launches;
+  // host-buffer path scratch (lazily allocated)
+  double* slab[kSlabs];
+  long long slab_cells;
+  cudaStream_t slab_stream[kSlabs];
+};
+
+extern "C" {
+
+const char* mgrhd_last_error(void) { return g_err; }
+
+int mgrhd_init(mgrhd_ctx** out, const double* edges, int Nq, const mgrhd_units* u,
+               const mgrhd_opacity_model* m) {
+  if (out) *out = nullptr;
+  if (!out || !edges || !u || !m || !m->kappa_lo || !m->alpha) return MGRHD_ERR_ARG;
+  if (Nq < 1 || Nq > MGRHD_MAX_GROUPS) return MGRHD_ERR_ARG;
+  if (m->closure < 0 || m->closure > 1 || m->spectrum != 0) return MGRHD_ERR_ARG;
+  if (m->outer_stop < 0 || m->outer_stop > 1 || m->newton_maxit < 1 || m->outer_maxit < 1)
+    return MGRHD_ERR_ARG;
+  if (!(u->a_rad > 0) || !(u->k_B > 0) || !(u->h_planck > 0) || !(u->mean_mass > 0) ||
+      !(u->gamma > 1) || !(m->newton_tol > 0) || !(m->outer_tol > 0))
+    return MGRHD_ERR_RANGE;
+  for (int g = 0; g < Nq; ++g) {
+    if (!(edges[g] >= 0.0) || !(edges[g + 1] > edges[g])) return MGRHD_ERR_EDGES;
+    if (m->alpha[g] != 0.0 && (edges[g] == 0.0 || std::isinf(edges[g + 1]))) return MGRHD_ERR_ALPHA;
+    if (!std::isfinite(m->alpha[g]) || !(m->kappa_lo[g] >= 0.0)) return MGRHD_ERR_RANGE;
+  }
+  mgrhd_ctx* ctx = new (std::nothrow) mgrhd_ctx();
+  if (!ctx) return MGRHD_ERR_ARG;
+  std::memset(ctx, 0, sizeof *ctx);
+  Params& P = ctx->P;
+  P.Nq = Nq;
+  P.closure = m->closure;
+  P.newton_maxit = m->newton_maxit;
+  P.outer_maxit = m->outer_maxit;
+  P.outer_stop = m->outer_stop;
+  P.newton_tol = m->newton_tol;
+  P.outer_tol = m->outer_tol;
+  P.outer_rel_tol = m->outer_rel_tol;
+  P.a_rad = u->a_rad;
+  P.h_over_k = u->h_planck / u->k_B;
+  P.cv_over_rho = u->k_B / ((u->gamma - 1.0) * u->mean_mass);
+  for (int g = 0; g <= Nq; ++g) P.nu[g] = edges[g];
+  for (int g = 0; g < Nq; ++g) {
+    const double a = m->alpha[g], k = m->kappa_lo[g];
+    P.alpha[g] = a;
+    P.k_lo[g] = k;
+    if (a == 0.0) {                       // piecewise constant, Eq. 17
+      P.k_hi[g] = k;
+      P.k_mean[g] = k;
+    } else {                              // Eq. 19 at nu_g+; Eq. 30 with alpha_Q = -1
+      const double z = a * std::log(edges[g + 1] / edges[g]);
+      P.k_hi[g] = k * std::exp(z);
+      P.k_mean[g] = k * (std::expm1(z) / z);
+    }
+    P.inv_k_mean[g] = 1.0 / P.k_mean[g];
+  }
+  cudaError_t e = cudaGetDevice(&ctx->device);
+  if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, ctx->device);
+  if (e == cudaSuccess) e = upload_tables_for_current_device();
+  if (e == cudaSuccess) e = cudaMalloc(&ctx->d_stats, kStatCount * sizeof(unsigned long long));
+  if (e == cudaSuccess) e = cudaMemset(ctx->d_stats, 0, kStatCount * sizeof(unsigned long long));
+  if (e != cudaSuccess) {
+    cuda_ok(e, "mgrhd_init");
+    if (ctx->d_stats) cudaFree(ctx->d_stats);
+    delete ctx;
+    return MGRHD_ERR_CUDA;
+  }
+  *out = ctx;
+  return MGRHD_OK;
+}
+
+static int check_call(const mgrhd_ctx* ctx, const mgrhd_state* s, long long n, double dt, double c,
+                      double chat) {
+  if (!ctx || !s || n < 0) return MGRHD_ERR_ARG;
+  if (!(dt > 0.0) || !(c > 0.0) || !(chat > 0.0) || chat > c) return MGRHD_ERR_RANGE;
+  if (n > 0 && (!s->rho || !s->mom[0] || !s->mom[1] || !s->mom[2] || !s->Egas || !s->Erad ||
+                !s->Frad[0] || !s->Frad[1] || !s->Frad[2]))
+    return MGRHD_ERR_ARG;
+  return MGRHD_OK;
+}
+
+static int launch_update(mgrhd_ctx* ctx, const StatePtrs& S, long long n, long long stride, double dt,
+                         double c, double chat, cudaStream_t st) {
+  Params P = ctx->P;
+  P.dt = dt; P.c = c; P.c_hat = chat; P.ncells = n; P.stride = stride;
+  long long blocks = (n + kBlock - 1) / kBlock;
+  const long long cap = (long long)ctx->sm_count * 64;
+  if (blocks > cap) blocks = cap;
+  const dim3 grid((unsigned)blocks), block(kBlock);
+  if (P.Nq <= 4) source_update_kernel<4><<<grid, block, 0, st>>>(P, S, ctx->d_stats);
+  else if (P.Nq <= 8) source_update_kernel<8><<<grid, block, 0, st>>>(P, S, ctx->d_stats);
+  else if (P.Nq <= 16) source_update_kernel<16><<<grid, block, 0, st>>>(P, S, ctx->d_stats);
+  else if (P.Nq <= 32) source_update_kernel<32><<<grid, block, 0, st>>>(P, S, ctx->d_stats);
+  else source_update_kernel<64><<<grid, block, 0, st>>>(P, S, ctx->d_stats);
+  ctx->launches++;
+  ctx->last_stream = st;
+  CU(cudaGetLastError());
+  return MGRHD_OK;
+}
+
+static StatePtrs to_ptrs(const mgrhd_state* s) {
+  StatePtrs S;
+  S.rho = s->rho;
+  for (int i = 0; i < 3; ++i) { S.mom[i] = s->mom[i]; S.Frad[i] = s->Frad[i]; }
+  S.Egas = s->Egas;
+  S.Erad = s->Erad;
+  S.kappa_scale = s->kappa_scale;
+  return S;
+}
+
+int mgrhd_source_update(mgrhd_ctx* ctx, const mgrhd_state* s, long long n, double dt, double c,
+                        double chat, void* stream) {
+  int rc = check_call(ctx, s, n, dt, c, chat);
+  if (rc != MGRHD_OK) return rc;
+  if (n == 0) return MGRHD_OK;
+  return launch_update(ctx, to_ptrs(s), n, n, dt, c, chat, (cudaStream_t)stream);
+}
+
+int mgrhd_conserved_totals(mgrhd_ctx* ctx, const mgrhd_state* s, long long n, double c, double chat,
+                           double* outE, double* outP, void* stream) {
+  int rc = check_call(ctx, s, n, 1.0, c, chat);
+  if (rc != MGRHD_OK) return rc;
+  if (!outE || !outP) return MGRHD_ERR_ARG;
+  if (n == 0) return MGRHD_OK;
+  long long blocks = (n + 255) / 256;
+  const long long cap = (long long)ctx->sm_count * 32;
+  if (blocks > cap) blocks = cap;
+  conserved_totals_kernel<<<(unsigned)blocks, 256, 0, (cudaStream_t)stream>>>(
+      to_ptrs(s), ctx->P.Nq, n, n, c, chat, outE, outP);
+  ctx->launches++;
+  ctx->last_stream = (cudaStream_t)stream;
+  CU(cudaGetLastError());
+  return MGRHD_OK;
+}
+
+int mgrhd_source_update_host(mgrhd_ctx* ctx, const mgrhd_state* s, long long n, double dt, double c,
+                             double chat) {
+  int rc = check_call(ctx, s, n, dt, c, chat);
+  if (rc != MGRHD_OK) return rc;
+  if (n == 0) return MGRHD_OK;
+  const int Nq = ctx->P.Nq;
+  const long long per_cell = 6 + 4ll * Nq;     // rho, mom[3], Egas, kappa_scale, Erad, Frad[3]
+  if (!ctx->slab[0]) {
+    long long sc = kSlabBytes / (8 * per_cell);
+    sc = (sc / 1024) * 1024;
+    if (sc < 1024) sc = 1024;
+    for (int j = 0; j < kSlabs; ++j) {
+      CU(cudaMalloc(&ctx->slab[j], (size_t)sc * per_cell * sizeof(double)));
+      CU(cudaStreamCreateWithFlags(&ctx->slab_stream[j], cudaStreamNonBlocking));
+    }
+    ctx->slab_cells = sc;
+  }
+  const long long sc = ctx->slab_cells;
+  const size_t pitch_h = (size_t)n * sizeof(double), pitch_d = (size_t)sc * sizeof(double);
+  int j = 0;
+  for (long long lo = 0; lo < n; lo += sc, j = (j + 1) % kSlabs) {
+    const long long m = (n - lo < sc) ? (n - lo) : sc;
+    const size_t w = (size_t)m * sizeof(double);
+    cudaStream_t st = ctx->slab_stream[j];
+    double* d = ctx->slab[j];
+    StatePtrs S;
+    double* q = d;
+    S.rho = q; q += sc;
+    for (int i = 0; i < 3; ++i) { S.mom[i] = q; q += sc; }
+    S.Egas = q; q += sc;
+    double* d_ks = q; q += sc;
+    S.kappa_scale = s->kappa_scale ? d_ks : nullptr;
+    S.Erad = q; q += sc * Nq;
+    for (int i = 0; i < 3; ++i) { S.Frad[i] = q; q += sc * Nq; }
+    // host -> device
+    CU(cudaMemcpyAsync((void*)S.rho, s->rho + lo, w, cudaMemcpyHostToDevice, st));
+    for (int i = 0; i < 3; ++i) CU(cudaMemcpyAsync(S.mom[i], s->mom[i] + lo, w, cudaMemcpyHostToDevice, st));
+    CU(cudaMemcpyAsync(S.Egas, s->Egas + lo, w, cudaMemcpyHostToDevice, st));
+    if (s->kappa_scale) CU(cudaMemcpyAsync(d_ks, s->kappa_scale + lo, w, cudaMemcpyHostToDevice, st));
+    CU(cudaMemcpy2DAsync(S.Erad, pitch_d, s->Erad + lo, pitch_h, w, Nq, cudaMemcpyHostToDevice, st));
+    for (int i = 0; i < 3; ++i)
+      CU(cudaMemcpy2DAsync(S.Frad[i], pitch_d, s->Frad[i] + lo, pitch_h, w, Nq, cudaMemcpyHostToDevice, st));
+    // update
+    rc = launch_update(ctx, S, m, sc, dt, c, chat, st);
+    if (rc != MGRHD_OK) return rc;
+    // device -> host (rho and kappa_scale are read only)
+    for (int i = 0; i < 3; ++i) CU(cudaMemcpyAsync(s->mom[i] + lo, S.mom[i], w, cudaMemcpyDeviceToHost, st));
+    CU(cudaMemcpyAsync(s->Egas + lo, S.Egas, w, cudaMemcpyDeviceToHost, st));
+    CU(cudaMemcpy2DAsync(s->Erad + lo, pitch_h, S.Erad, pitch_d, w, Nq, cudaMemcpyDeviceToHost, st));
+    for (int i = 0; i < 3; ++i)
+      CU(cudaMemcpy2DAsync(s->Frad[i] + lo, pitch_h, S.Frad[i], pitch_d, w, Nq, cudaMemcpyDeviceToHost, st));
+  }
+  for (int k = 0; k < kSlabs; ++k) CU(cudaStreamSynchronize(ctx->slab_stream[k]));
+  return MGRHD_OK;
+}
+
+int mgrhd_get_stats(mgrhd_ctx* ctx, mgrhd_stats* out) {
+  if (!ctx || !out) return MGRHD_ERR_ARG;
+  if (ctx->slab[0]) for (int k = 0; k < kSlabs; ++k) CU(cudaStreamSynchronize(ctx->slab_stream[k]));
+  CU(cudaStreamSynchronize(ctx->last_stream));
+  unsigned long long h[kStatCount];
+  CU(cudaMemcpy(h, ctx->d_stats, sizeof h, cudaMemcpyDeviceToHost));
+  out->n_cells = (long long)h[kStatCells];
+  out->n_newton_unconverged = (long long)h[kStatNewtonUnconv];
+  out->n_outer_unconverged = (long long)h[kStatOuterUnconv];
+  out->n_T_nonpositive_steps = (long long)h[kStatTNonPos];
+  out->n_chiF_guard = (long long)h[kStatChiFGuard];
+  out->n_denominator_nonpositive = (long long)h[kStatDenNonPos];
+  out->newton_evals_total = (long long)h[kStatNewtonEvals];
+  out->outer_trips_total = (long long)h[kStatOuterTrips];
+  for (int b = 0; b < MGRHD_HIST; ++b) {
+    out->newton_hist[b] = (long long)h[kStatNewtonHist + b];
+    out->outer_hist[b] = (long long)h[kStatOuterHist + b];
+  }
+  return MGRHD_OK;
+}
+
+int mgrhd_reset_stats(mgrhd_ctx* ctx) {
+  if (!ctx) return MGRHD_ERR_ARG;
+  CU(cudaMemsetAsync(ctx->d_stats, 0, kStatCount * sizeof(unsigned long long), ctx->last_stream));
+  return MGRHD_OK;
+}
+
+long long mgrhd_launch_count(const mgrhd_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+int mgrhd_measure_dfma_peak(long long iters, double* fma_per_second) {
+  if (!fma_per_second || iters < 8) return MGRHD_ERR_ARG;
+  int dev = 0, sms = 0;
+  CU(cudaGetDevice(&dev));
+  CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  double* d_out = nullptr;
+  CU(cudaMalloc(&d_out, sizeof(double)));
+  cudaEvent_t e0, e1;
+  CU(cudaEventCreate(&e0));
+  CU(cudaEventCreate(&e1));
+  const int blocks = sms * 8, threads = 256;
+  iters = (iters / 8) * 8;
+  dfma_peak_kernel<<<blocks, threads>>>(iters / 16, d_out);   // warm-up
+  float best = 1e30f;
+  for (int r = 0; r < 3; ++r) {
+    CU(cudaEventRecord(e0));
+    dfma_peak_kernel<<<blocks, threads>>>(iters, d_out);
+    CU(cudaEventRecord(e1));
+    CU(cudaEventSynchronize(e1));
+    float ms = 0.f;
+    CU(cudaEventElapsedTime(&ms, e0, e1));
+    if (ms < best) best = ms;
+  }
+  CU(cudaGetLastError());
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  cudaFree(d_out);
+  *fma_per_second = (double)blocks * threads * (double)iters / (best * 1e-3);
+  return MGRHD_OK;
+}
+
+void mgrhd_free(mgrhd_ctx* ctx) {
+  if (!ctx) return;
+  for (int k = 0; k < kSlabs; ++k) {
+    if (ctx->slab[k]) cudaFree(ctx->slab[k]);
+    if (ctx->slab_stream[k]) cudaStreamDestroy(ctx->slab_stream[k]);
+  }
+  if (ctx->d_stats) cudaFree(ctx->d_stats);
+  delete ctx;
+}
+
+}  // extern "C"

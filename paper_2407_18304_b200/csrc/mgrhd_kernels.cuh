@@ -1,0 +1,292 @@
+// mgrhd_kernels.cuh -- the per-cell implicit source update (Eq. 37-52)
+// as a CUDA kernel: one thread owns one cell from load to store.
+//
+// Why thread-per-cell: the dominant cost is the Planck edge functions at the Nq+1 group
+// edges, re-evaluated at every trial temperature.  With one cell per thread the EDGE index is
+// warp-uniform, so the 32 lanes evaluate the same edge at 32 temperatures and almost always
+// fall in the same branch of planck_edge(); with lanes mapped to groups every warp would
+// execute every branch.  See DESIGN.md "Kernel mapping".
+//
+// Product code; shares nothing with oracle/.
+#pragma once
+#include "mgrhd_planck.cuh"
+
+namespace mgrhd {
+
+__device__ __forceinline__ double norm3(double a, double b, double c) {
+  return sqrt(a * a + b * b + c * c);
+}
+
+// v^j P^{ji} for one group (closure reading S7 of DESIGN.md): Levermore/M1
+// or Eddington P = E/3 I.
+__device__ __forceinline__ void closure_vP(int closure, double E, double F0, double F1, double F2,
+                                           double v0, double v1, double v2, double c,
+                                           double& p0, double& p1, double& p2) {
+  const double Fn = norm3(F0, F1, F2);
+  if (closure == 1 || !(E > 0.0) || Fn == 0.0) {
+    const double t = E / 3.0;
+    p0 = t * v0; p1 = t * v1; p2 = t * v2;
+    return;
+  }
+  double f = Fn / (c * E);
+  if (f > 1.0) f = 1.0;
+  const double chi = (3.0 + 4.0 * f * f) / (5.0 + 2.0 * sqrt(4.0 - 3.0 * f * f));
+  const double n0 = F0 / Fn, n1 = F1 / Fn, n2 = F2 / Fn;
+  const double ndv = n0 * v0 + n1 * v1 + n2 * v2;
+  const double a = 0.5 * (1.0 - chi), b = 0.5 * (3.0 * chi - 1.0) * ndv;
+  p0 = E * (a * v0 + b * n0);
+  p1 = E * (a * v1 + b * n1);
+  p2 = E * (a * v2 + b * n2);
+}
+
+// MAXQ: compile-time bound on Nq (per-thread group arrays are sized MAXQ).
+template <int MAXQ>
+__global__ void __launch_bounds__(128)
+source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ StatePtrs S,
+                     unsigned long long* __restrict__ stats) {
+  __shared__ unsigned int s_hist[2 * MGRHD_HIST];
+  for (int t = threadIdx.x; t < 2 * MGRHD_HIST; t += blockDim.x) s_hist[t] = 0u;
+  __syncthreads();
+
+  const int Nq = P.Nq;
+  const long long n = P.ncells, stride = P.stride;
+  const double dt = P.dt, c = P.c, chat = P.c_hat;
+  const double c_over_chat = c / chat;
+
+  unsigned int cnt_newton_unconv = 0, cnt_outer_unconv = 0, cnt_Tnonpos = 0, cnt_guard = 0,
+               cnt_den = 0, cnt_evals = 0, cnt_trips = 0, cnt_cells = 0;
+
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n;
+       i += (long long)gridDim.x * blockDim.x) {
+    // ---- a0: load and derive (Eq. 34, Eq. 50) ---------------------------------------
+    double Et[MAXQ], R[MAXQ], vF[MAXQ], Fk0[MAXQ], Fk1[MAXQ], Fk2[MAXQ];
+    double Ag[MAXQ];     // chi_B Bt_g - D_g/3 at the last evaluated T (Eq. 51 source)
+    double chiFg[MAXQ];  // chi_F,g at the last evaluated T (Eq. 27)
+    double da[MAXQ], db[MAXQ];  // Newton step pieces: dR_g = da + db*dx0
+
+    const double rho = S.rho[i];
+    const double ks = S.kappa_scale ? S.kappa_scale[i] : 1.0;
+    const double chis = rho * ks;                 // chi_{g-} = chis * k_lo[g]
+    const double inv_chis = 1.0 / chis;
+    const double momt0 = S.mom[0][i], momt1 = S.mom[1][i], momt2 = S.mom[2][i];
+    const double Egas_t = S.Egas[i];
+    const double Cv = rho * P.cv_over_rho;
+
+    double sumEt = 0.0;
+    for (int g = 0; g < Nq; ++g) {
+      const long long o = (long long)g * stride + i;
+      Et[g] = S.Erad[o];
+      Fk0[g] = S.Frad[0][o];
+      Fk1[g] = S.Frad[1][o];
+      Fk2[g] = S.Frad[2][o];
+      R[g] = 0.0;
+      sumEt += Et[g];
+    }
+    const double Etot = Egas_t + (chat / c) * sumEt;   // Eq. 50 as printed, S_g = 0
+
+    double momk0 = momt0, momk1 = momt1, momk2 = momt2;
+    double momn0 = momt0, momn1 = momt1, momn2 = momt2;
+    double Egs = Egas_t, Egas_new = Egas_t;
+    int evals = 0, trips = 0;
+
+    // lagged work-term factor v.F_g for the first trip
+    {
+      const double v0 = momk0 / rho, v1 = momk1 / rho, v2 = momk2 / rho;
+      for (int g = 0; g < Nq; ++g) vF[g] = v0 * Fk0[g] + v1 * Fk1[g] + v2 * Fk2[g];
+    }
+
+    for (int k = 0; k < P.outer_maxit; ++k) {
+      // ---- O1: lagged velocity ------------------------------------------------------
+      const double v0 = momk0 / rho, v1 = momk1 / rho, v2 = momk2 / rho;
+      const double Ekin = (momk0 * momk0 + momk1 * momk1 + momk2 * momk2) / (2.0 * rho);
+      if (!((Egs - Ekin) / Cv > 0.0)) { cnt_Tnonpos++; break; }
+
+      // ---- inner Newton-Raphson on x = (E_gas, R_1..R_Nq), PAPER.md:393-451 ----------
+      for (int it = 0;; ++it) {
+        const double T = (Egs - Ekin) / Cv;
+        const double T2 = T * T;
+        const double aT4 = P.a_rad * T2 * T2;
+        const double beta = P.h_over_k / T;
+        double sumR = 0.0, sumAbsFR = 0.0, S1 = 0.0, S2 = 0.0;
+        EdgeFn lo = planck_edge(P.nu[0] * beta);
+        if (P.nu[0] == 0.0) { lo.yz = 0.0; lo.xi = 0.0; lo.small = true; }
+        for (int g = 0; g < Nq; ++g) {
+          // a1: edge functions at the upper edge of group g
+          const double nuh = P.nu[g + 1];
+          EdgeFn hi = planck_edge(nuh * beta);
+          // a2: group Planck integral and Doppler boundary terms (Eq. 11, 18, 22)
+          const double chi_lo = chis * P.k_lo[g], chi_hi = chis * P.k_hi[g];
+          const double chiE = chis * P.k_mean[g];            // = chi_B (alpha_Q = -1 for both)
+          const double Bt = aT4 * planck_dY(lo, hi);
+          const double Db = aT4 * (hi.xi - lo.xi);
+          const double D = aT4 * (chi_hi * hi.xi - chi_lo * lo.xi);
+          const double dBdT = (4.0 * Bt - Db) / T;
+          // a3: flux-mean opacity, Eq. 27, with the Wien-limit guard (S8)
+          const double alpha = P.alpha[g];
+          const double den = (4.0 / 3.0) * Bt - Db / 3.0;
+          double chiF;
+          if (!(den >= 1e-280 * aT4) || isinf(den)) {
+            chiF = chi_lo;
+            if (evals == 0) cnt_guard++;
+          } else {
+            chiF = ((chiE + chiE / 3.0) * Bt + (alpha * chiE * Bt - D) / 3.0) / den;
+          }
+          if (!(1.0 + chat * chiF * dt > 0.0)) {
+            if (evals == 0) cnt_den++;
+            chiF = chiE;
+          }
+          // a4: residuals (Eq. 41, 42 solved for E_g)
+          const double inv_chiE = inv_chis * P.inv_k_mean[g];
+          const double W = (1.0 + alpha) * chiF * vF[g] / c;
+          const double itau = inv_chiE / (chat * dt);        // 1/(c_hat dt chi_E)
+          const double Eg = Bt + W * inv_chiE / c - R[g] * itau;
+          const double FR = Eg - Et[g] - R[g];
+          sumR += R[g];
+          sumAbsFR += fabs(FR);
+          // a5: Jacobian pieces (Eq. 44-47) folded into the arrowhead elimination (Eq. 48)
+          const double Jg0 = dBdT / Cv;
+          const double inv_Jgg = -1.0 / (itau + 1.0);
+          S1 += c_over_chat * FR * inv_Jgg;
+          S2 += c_over_chat * Jg0 * inv_Jgg;
+          da[g] = -FR * inv_Jgg;
+          db[g] = -Jg0 * inv_Jgg;
+          Ag[g] = chiE * Bt - D / 3.0;
+          chiFg[g] = chiF;
+          lo = hi;
+        }
+        const double FG = Egs - Egas_t + c_over_chat * sumR;
+        evals++;
+        // Eq. 49
+        if (fabs(FG) / Etot < P.newton_tol && c_over_chat * sumAbsFR / Etot < P.newton_tol) break;
+        if (it >= P.newton_maxit) { cnt_newton_unconv++; break; }
+        // eliminate the gas row: dx0 = (-F_G + sum J0g F_R,g/Jgg) / (1 - sum J0g Jg0/Jgg)
+        const double dx0 = (-FG + S1) / (1.0 - S2);
+        double lam = 1.0;
+        for (int h = 0; h < 10 && !((Egs + lam * dx0 - Ekin) / Cv > 0.0); ++h) {
+          lam *= 0.5;
+          cnt_Tnonpos++;
+        }
+        Egs += lam * dx0;
+        for (int g = 0; g < Nq; ++g) R[g] += lam * (da[g] + db[g] * dx0);
+      }
+
+      // ---- a6: energy commit -----------------------------------------
+      double sumR = 0.0;
+      for (int g = 0; g < Nq; ++g) sumR += R[g];
+      Egas_new = Egas_t - c_over_chat * sumR;
+
+      // ---- a7: closure + flux update (Eq. 51); a8: gas momentum (Eq. 52) ------------
+      double dF0 = 0.0, dF1 = 0.0, dF2 = 0.0;
+      bool rel_ok = true;
+      for (int g = 0; g < Nq; ++g) {
+        const long long o = (long long)g * stride + i;
+        const double Ft0 = S.Frad[0][o], Ft1 = S.Frad[1][o], Ft2 = S.Frad[2][o];
+        const double Enew = Et[g] + R[g];
+        double p0, p1, p2;
+        closure_vP(P.closure, Enew, Fk0[g], Fk1[g], Fk2[g], v0, v1, v2, c, p0, p1, p2);
+        const double chiE = chis * P.k_mean[g];
+        const double w = (1.0 + P.alpha[g]) * chiE;
+        const double inv_den = 1.0 / (1.0 + chat * chiFg[g] * dt);
+        const double A = Ag[g];
+        const double Fn0 = (Ft0 + chat * dt * (v0 * A + w * p0)) * inv_den;
+        const double Fn1 = (Ft1 + chat * dt * (v1 * A + w * p1)) * inv_den;
+        const double Fn2 = (Ft2 + chat * dt * (v2 * A + w * p2)) * inv_den;
+        dF0 += Fn0 - Ft0; dF1 += Fn1 - Ft1; dF2 += Fn2 - Ft2;
+        if (P.outer_stop == 1) {
+          const double d = norm3(Fn0 - Fk0[g], Fn1 - Fk1[g], Fn2 - Fk2[g]);
+          if (!(d <= P.outer_rel_tol * norm3(Fn0, Fn1, Fn2))) rel_ok = false;
+        }
+        Fk0[g] = Fn0; Fk1[g] = Fn1; Fk2[g] = Fn2;
+      }
+      const double icc = 1.0 / (c * chat);
+      momn0 = momt0 - dF0 * icc; momn1 = momt1 - dF1 * icc; momn2 = momt2 - dF2 * icc;
+      trips++;
+
+      // ---- a9: outer convergence (reading S10) ------------------------
+      const double vn0 = momn0 / rho, vn1 = momn1 / rho, vn2 = momn2 / rho;
+      double dW = 0.0, sumAbsR = 0.0;
+      for (int g = 0; g < Nq; ++g) {
+        const double vFn = vn0 * Fk0[g] + vn1 * Fk1[g] + vn2 * Fk2[g];
+        const double wf = (1.0 + P.alpha[g]) * chiFg[g] / c;
+        dW += fabs(wf * vFn - wf * vF[g]);
+        sumAbsR += fabs(R[g]);
+        vF[g] = vFn;                                   // lagged v.F_g of the next trip
+      }
+      if (P.outer_stop == 1) {
+        const double d = norm3(momn0 - momk0, momn1 - momk1, momn2 - momk2);
+        if (!(d <= P.outer_rel_tol * norm3(momn0, momn1, momn2))) rel_ok = false;
+      }
+      const double delta = dW * (chat / c) * dt;
+      if (delta <= P.outer_tol * fmax(sumAbsR, Etot) && rel_ok) break;
+      if (k == P.outer_maxit - 1) { cnt_outer_unconv++; break; }
+      momk0 = momn0; momk1 = momn1; momk2 = momn2;
+    }
+
+    // ---- a10: store -------------------------------------------------------------------
+    if (trips > 0) {
+      S.mom[0][i] = momn0; S.mom[1][i] = momn1; S.mom[2][i] = momn2;
+      S.Egas[i] = Egas_new;   // total gas energy; E_int = Egas - |mom|^2/(2 rho)
+      for (int g = 0; g < Nq; ++g) {
+        const long long o = (long long)g * stride + i;
+        S.Erad[o] = Et[g] + R[g];
+        S.Frad[0][o] = Fk0[g];
+        S.Frad[1][o] = Fk1[g];
+        S.Frad[2][o] = Fk2[g];
+      }
+    }
+    cnt_evals += evals;
+    cnt_trips += trips;
+    cnt_cells++;
+    atomicAdd(&s_hist[evals < MGRHD_HIST ? evals : MGRHD_HIST - 1], 1u);
+    atomicAdd(&s_hist[MGRHD_HIST + (trips < MGRHD_HIST ? trips : MGRHD_HIST - 1)], 1u);
+  }
+
+  // ---- diagnostics: warp-reduce the scalar counters, one atomic per warp ------------------
+  unsigned int vals[8] = {cnt_cells, cnt_newton_unconv, cnt_outer_unconv, cnt_Tnonpos,
+                          cnt_guard, cnt_den, cnt_evals, cnt_trips};
+#pragma unroll
+  for (int s = 0; s < 8; ++s) {
+    unsigned int v = vals[s];
+    for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
+    if ((threadIdx.x & 31) == 0 && v) atomicAdd(&stats[s], (unsigned long long)v);
+  }
+  __syncthreads();
+  for (int t = threadIdx.x; t < 2 * MGRHD_HIST; t += blockDim.x)
+    if (s_hist[t]) atomicAdd(&stats[kStatNewtonHist + t], (unsigned long long)s_hist[t]);
+}
+
+// Per-cell conserved totals: E_gas + (c/c_hat) sum E_g and
+// rho v + (c c_hat)^-1 sum F_g.
+__global__ void conserved_totals_kernel(const __grid_constant__ StatePtrs S, int Nq, long long n,
+                                        long long stride, double c, double chat,
+                                        double* __restrict__ outE, double* __restrict__ outP) {
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n;
+       i += (long long)gridDim.x * blockDim.x) {
+    double sE = 0.0, s0 = 0.0, s1 = 0.0, s2 = 0.0;
+    for (int g = 0; g < Nq; ++g) {
+      const long long o = (long long)g * stride + i;
+      sE += S.Erad[o];
+      s0 += S.Frad[0][o]; s1 += S.Frad[1][o]; s2 += S.Frad[2][o];
+    }
+    const double icc = 1.0 / (c * chat);
+    outE[i] = S.Egas[i] + (c / chat) * sE;
+    outP[i] = S.mom[0][i] + icc * s0;
+    outP[n + i] = S.mom[1][i] + icc * s1;
+    outP[2 * n + i] = S.mom[2][i] + icc * s2;
+  }
+}
+
+// Dependency-free DFMA throughput probe: 8 independent chains per thread.
+__global__ void dfma_peak_kernel(long long iters, double* out) {
+  double a0 = threadIdx.x * 1e-9, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5,
+         a6 = a0 + 6, a7 = a0 + 7;
+  const double m = 0.999999, b = 1e-7;
+  for (long long k = 0; k < iters; k += 8) {
+    a0 = fma(a0, m, b); a1 = fma(a1, m, b); a2 = fma(a2, m, b); a3 = fma(a3, m, b);
+    a4 = fma(a4, m, b); a5 = fma(a5, m, b); a6 = fma(a6, m, b); a7 = fma(a7, m, b);
+  }
+  const double s = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
+  if (s == 123.456) out[0] = s;  // never true; keeps the chains alive
+}
+
+}  // namespace mgrhd

@@ -1,0 +1,71 @@
+// mgrhd_params.h -- launch-time parameter block shared by the host API (mgrhd_api.cu) and
+// the device kernels (mgrhd_kernels.cuh).  Passed BY VALUE as a __grid_constant__ kernel
+// argument, so it lives in the constant bank: every table read below with a warp-uniform
+// index is a uniform constant load, and several contexts can run concurrently on different
+// streams without sharing a __constant__ symbol.
+//
+// Product code.  Shares nothing with oracle/.
+#pragma once
+#include "../../include/mgrhd.h"
+
+namespace mgrhd {
+
+constexpr int kMaxG = MGRHD_MAX_GROUPS;
+constexpr int kSmallTerms = 16;   // even Maclaurin terms kept in the small-x edge functions
+constexpr int kSeriesMax = 40;    // longest exponential series (x >= kXSplit)
+
+// Device counters, one block of long long in global memory (see mgrhd_stats).
+enum StatSlot {
+  kStatCells = 0,
+  kStatNewtonUnconv,
+  kStatOuterUnconv,
+  kStatTNonPos,
+  kStatChiFGuard,
+  kStatDenNonPos,
+  kStatNewtonEvals,
+  kStatOuterTrips,
+  kStatNewtonHist,                       // MGRHD_HIST slots
+  kStatOuterHist = kStatNewtonHist + MGRHD_HIST,
+  kStatCount = kStatOuterHist + MGRHD_HIST
+};
+
+struct Params {
+  // ---- group structure and opacity table (set once by mgrhd_init) -------------------
+  int Nq;
+  int closure;        // 0 Levermore/M1, 1 Eddington
+  int newton_maxit, outer_maxit, outer_stop;
+  double newton_tol, outer_tol, outer_rel_tol;
+  double a_rad;
+  double h_over_k;    // h / k_B : x_e = nu_e * h_over_k / T
+  double cv_over_rho; // k_B / ((gamma-1) mean_mass)
+  double nu[kMaxG + 1];     // group edges; nu[0] may be 0, nu[Nq] may be +inf
+  double alpha[kMaxG];      // alpha_{chi0,g}
+  double k_lo[kMaxG];       // kappa_lo[g]                       (chi_{g-} = rho*scale*k_lo)
+  double k_hi[kMaxG];       // kappa_lo[g] * r_g^alpha_g         (chi_{g+}, Eq. 19 at nu_g+)
+  double k_mean[kMaxG];     // kappa_lo[g] * (r^alpha-1)/(alpha ln r)   (Eq. 30 with alpha_Q=-1)
+  double inv_k_mean[kMaxG]; // 1 / k_mean[g]
+  // ---- per call ------------------------------------------------------------------
+  double dt, c, c_hat;
+  long long ncells;   // cells in this launch
+  long long stride;   // distance (in doubles) between consecutive groups in Erad/Frad
+};
+
+struct StatePtrs {
+  const double* rho;
+  double* mom[3];
+  double* Egas;
+  double* Erad;
+  double* Frad[3];
+  const double* kappa_scale;  // may be null
+};
+
+// Small-x Maclaurin tables, filled by the host at first use (mgrhd_api.cu: fill_planck_tables)
+// and uploaded to __constant__ memory in the kernel translation unit.
+struct PlanckTables {
+  // t/(e^t-1) = 1 - t/2 + sum_{n>=1} b2n[n-1] t^(2n);  b_{2n} = B_{2n}/(2n)!
+  double xi_c[kSmallTerms];   // b_{2n}                     : Xi(x) = C x^3 (1 - x/2 + sum xi_c[n-1] x^(2n))
+  double y_c[kSmallTerms];    // b_{2n} / (2n+3)            : Y(x)  = C x^3 (1/3 - x/8 + sum y_c[n-1] x^(2n))
+  double inv_n[kSeriesMax + 1];  // 1/n, n = 1..kSeriesMax (index 0 unused)
+};
+
+}  // namespace mgrhd

@@ -1,0 +1,72 @@
+"""Shared helpers of the GPU parity tests: run the oracle and the CUDA path on the same seeded
+host state and compare element by element with the tolerance of DESIGN.md (reading S14):
+
+    |gpu - ref| <= 1e-10 |ref| + 1e-14 S_cell
+    S_cell = E_tot (energies), c E_tot (fluxes), |rho v| + sum_g |F_g|/(c c_hat) (momentum)
+
+The 1e-10 is BASELINE.json north_star's "relative 1e-10 per field (FP64)"; the absolute floor
+is needed because Eq. 49 converges relative to E_tot, so groups holding 1e-300 of the energy
+are only as converged as T is.
+"""
+import numpy as np
+
+RTOL = 1e-10
+AFLOOR = 1e-14
+
+
+def oracle_model(oracle, wl, **kw):
+    args = dict(a_rad=wl.a_rad, k_B=wl.k_B, h_planck=wl.h_planck, mean_mass=wl.mean_mass, gamma=wl.gamma,
+                closure=wl.closure, newton_tol=wl.newton_tol, newton_maxit=wl.newton_maxit,
+                outer_maxit=wl.outer_maxit, outer_tol=wl.outer_tol, outer_stop=wl.outer_stop,
+                outer_rel_tol=wl.outer_rel_tol)
+    args.update(kw)
+    return oracle.OracleModel(wl.edges, wl.kappa_lo, wl.alpha, **args)
+
+
+def conserved(st, c, c_hat):
+    """Per-cell E_gas + (c/c_hat) sum E_g and rho v + sum F_g/(c c_hat)."""
+    E = st["Egas"] + (c / c_hat) * st["Erad"].sum(0)
+    P = st["mom"] + st["Frad"].sum(1) / (c * c_hat)
+    return E, P
+
+
+def scales(st0, c, c_hat):
+    Etot = st0["Egas"] + (c_hat / c) * st0["Erad"].sum(0)
+    Fn = np.sqrt((st0["Frad"] ** 2).sum(0))                       # [Nq, n]
+    Ps = np.sqrt((st0["mom"] ** 2).sum(0)) + Fn.sum(0) / (c * c_hat)
+    return Etot, Ps
+
+
+def compare(ref, got, st0, c, c_hat):
+    """Returns {field: (n_bad, worst excess ratio)}; excess ratio = |d| / allowed."""
+    Etot, Ps = scales(st0, c, c_hat)
+    out = {}
+    for key, S in (("Egas", Etot), ("Erad", Etot[None, :]), ("Frad", (c * Etot)[None, None, :]),
+                   ("mom", Ps[None, :])):
+        d = np.abs(got[key] - ref[key])
+        allowed = RTOL * np.abs(ref[key]) + AFLOOR * S
+        bad = ~(d <= allowed)                                      # NaN counts as bad
+        with np.errstate(invalid="ignore", divide="ignore"):
+            ratio = np.where(allowed > 0, d / allowed, np.where(d == 0, 0.0, np.inf))
+        out[key] = (int(bad.sum()), float(np.nanmax(ratio)) if ratio.size else 0.0)
+    return out
+
+
+def assert_parity(ref, got, st0, c, c_hat, label=""):
+    res = compare(ref, got, st0, c, c_hat)
+    bad = {k: v for k, v in res.items() if v[0] > 0}
+    assert not bad, f"{label} parity failed (field: (count, worst |d|/allowed)): {bad}; all: {res}"
+    return res
+
+
+def conservation_residual(st0, st1, c, c_hat):
+    """max over cells of |Delta(E_gas + (c/c_hat) sum E_g)|/E_scale and the same for momentum."""
+    E0, P0 = conserved(st0, c, c_hat)
+    E1, P1 = conserved(st1, c, c_hat)
+    Es = np.abs(st0["Egas"]) + (c / c_hat) * np.abs(st0["Erad"]).sum(0)
+    Ps = np.sqrt((st0["mom"] ** 2).sum(0)) + np.sqrt((st0["Frad"] ** 2).sum(0)).sum(0) / (c * c_hat)
+    rE = float(np.max(np.abs(E1 - E0) / Es))
+    dP = np.sqrt(((P1 - P0) ** 2).sum(0))
+    with np.errstate(invalid="ignore", divide="ignore"):
+        rP = float(np.max(np.where(Ps > 0, dP / Ps, dP)))
+    return rE, rP
