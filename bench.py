@@ -1,0 +1,405 @@
+"""bench.py -- throughput of mgrhd_source_update on the BASELINE.json workloads.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload 1..5] [--impl ours|reference]
+
+One "step" = one mgrhd_source_update over the whole workload (all SURVEY section 8(a) rows:
+load, Newton/outer iterations, store), starting from the same pristine state every step (the
+restore is a device-to-device copy outside the timed events; it also evicts L2).  Default
+workload: config 4 (256^3 cells, Nq=32, "rapidly variable opacity"), the one north_star's
+target is quoted on.  Prints ONE JSON line.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "source-update cell-groups/sec (FP64)"
+UNIT = "cell-groups/s"
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", type=int, default=4, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--cells", type=int, default=None, help="override the workload's cell count (debugging)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--cpu-sample-cells", type=int, default=None)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def workload_label(wl) -> str:
+    return f"config{wl.index}:{wl.name}"
+
+
+# --------------------------------------------------------------------------------------
+# clocks: sampled through NVML while the timed region runs
+# --------------------------------------------------------------------------------------
+class ClockSampler:
+    REASONS = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown",
+               0x40: "hw_thermal_slowdown", 0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting"}
+
+    def __init__(self, index: int):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thread = None
+        try:
+            import pynvml
+
+            pynvml.nvmlInit()
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+            phys = int(vis.split(",")[index]) if vis and vis.split(",")[index].isdigit() else index
+            self._h = pynvml.nvmlDeviceGetHandleByIndex(phys)
+            self._nv = pynvml
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self._nv = None
+
+    def _run(self):
+        nv = self._nv
+        while not self._stop.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self._h, nv.NVML_CLOCK_SM))
+                mask = nv.nvmlDeviceGetCurrentClocksEventReasons(self._h)
+                for bit, name in self.REASONS.items():
+                    if mask & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            self._stop.wait(0.02)
+
+    def start(self):
+        if self._nv is not None:
+            self._thread = threading.Thread(target=self._run, daemon=True)
+            self._thread.start()
+
+    def stop(self) -> dict:
+        self._stop.set()
+        if self._thread is not None:
+            self._thread.join()
+        return {"sm_mhz": statistics.median(self.samples) if self.samples else None,
+                "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+# --------------------------------------------------------------------------------------
+# CPU oracle legs (the only places bench.py touches oracle/)
+# --------------------------------------------------------------------------------------
+def oracle_model(oracle, wl):
+    return oracle.OracleModel(wl.edges, wl.kappa_lo, wl.alpha, a_rad=wl.a_rad, k_B=wl.k_B, h_planck=wl.h_planck,
+                              mean_mass=wl.mean_mass, gamma=wl.gamma, closure=wl.closure, newton_tol=wl.newton_tol,
+                              newton_maxit=wl.newton_maxit, outer_maxit=wl.outer_maxit, outer_tol=wl.outer_tol,
+                              outer_stop=wl.outer_stop, outer_rel_tol=wl.outer_rel_tol)
+
+
+def default_cpu_sample(wl) -> int:
+    """Cells the single-threaded oracle (dense LU, O(Nq^3) per Newton step) finishes in roughly 10-20 s."""
+    return {1: 65536, 2: 65536, 3: 32768, 4: 16384, 5: 4096}[wl.index]
+
+
+def time_oracle(wl, host_state: dict, dt: float) -> tuple[float, dict]:
+    """Seconds for one oracle update of host_state (in place) on one host core, and its stats."""
+    import oracle
+
+    oracle.build()
+    m = oracle_model(oracle, wl)
+    t0 = time.perf_counter()
+    st = oracle.source_update(m, host_state, dt, wl.c, wl.c_hat)
+    return time.perf_counter() - t0, st
+
+
+def run_reference(args) -> None:
+    """--impl reference: the oracle as it stands, on the host, on a bounded sample per step."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from paper_2407_18304_b200 import workloads as W
+
+    wl = W.workload(args.workload, ncells=args.cells)
+    sample = min(wl.ncells, args.cpu_sample_cells or max(1024, default_cpu_sample(wl) // 4))
+    st0 = W.to_numpy(wl.make_state(ncells=sample))
+    times = []
+    for step in range(args.warmup + args.steps):
+        st = {k: (None if v is None else v.copy()) for k, v in st0.items()}
+        dt, _ = time_oracle(wl, st, wl.dt_of_call(0))
+        if step >= args.warmup:
+            times.append(dt)
+    total = sum(times)
+    value = sample * wl.Nq * args.steps / total
+    desc = f"first {sample} cells of {workload_label(wl)} per step, single thread, dense LU"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_label(wl), "cells": sample, "Nq": wl.Nq},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+# --------------------------------------------------------------------------------------
+# our arm
+# --------------------------------------------------------------------------------------
+def alloc_like(state: dict, pin: bool = False) -> dict:
+    import torch
+
+    out = {}
+    for k, v in state.items():
+        if v is None:
+            out[k] = None
+        elif pin:
+            out[k] = torch.empty(v.shape, dtype=v.dtype, pin_memory=True)
+        else:
+            out[k] = torch.empty_like(v)
+    return out
+
+
+def copy_state(dst: dict, src: dict, non_blocking: bool = False) -> None:
+    for k, v in src.items():
+        if v is not None:
+            dst[k].copy_(v, non_blocking=non_blocking)
+
+
+def state_nbytes(state: dict, keys=None) -> int:
+    return sum(v.numel() * 8 for k, v in state.items() if v is not None and (keys is None or k in keys))
+
+
+def run_ours(args) -> None:
+    import torch
+    import torch.distributed as dist
+
+    from paper_2407_18304_b200 import binding, build, workloads as W
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if rank == 0:
+        build.build()
+    if world > 1:
+        dist.barrier()
+    binding.load_library()
+
+    wl = W.workload(args.workload, ncells=args.cells)
+    n, Nq = wl.ncells, wl.Nq
+    dt = wl.dt_of_call(0)
+    # weak scaling: every rank updates its own n cells (disjoint seeded cell ranges); no collective on the data path
+    pristine = wl.make_state(device="cuda", cell_start=rank * n, ncells=n)
+    work = alloc_like(pristine)
+    ctx = binding.Context.from_workload(wl)
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- conservation + iteration statistics + algorithmic flops: one untimed instrumented pass -------
+    E0 = torch.empty(n, dtype=torch.float64, device="cuda")
+    P0 = torch.empty(3, n, dtype=torch.float64, device="cuda")
+    E1, P1 = torch.empty_like(E0), torch.empty_like(P0)
+    copy_state(work, pristine)
+    ctx.conserved_totals(work, wl.c, wl.c_hat, E0, P0)
+    ctx.set_flop_counting(True)
+    ctx.reset_stats()
+    ctx.source_update(work, dt, wl.c, wl.c_hat)
+    stats = ctx.get_stats()
+    ctx.set_flop_counting(False)
+    ctx.conserved_totals(work, wl.c, wl.c_hat, E1, P1)
+    Es = pristine["Egas"].abs() + (wl.c / wl.c_hat) * pristine["Erad"].abs().sum(0)
+    resE = float(((E1 - E0).abs() / Es).max())
+    Ps = pristine["mom"].pow(2).sum(0).sqrt() + pristine["Frad"].pow(2).sum(0).sqrt().sum(0) / (wl.c * wl.c_hat)
+    dP = (P1 - P0).pow(2).sum(0).sqrt()
+    resP = float(torch.where(Ps > 0, dP / Ps, dP).max())
+    finite = all(bool(torch.isfinite(work[k]).all()) for k in ("mom", "Egas", "Erad", "Frad"))
+    del E0, P0, E1, P1, Es, Ps, dP
+    flops_per_launch = float(stats["flops"])
+
+    # ---- timed region: W warm-up + K timed steps, CUDA events on the launch stream ---------------------
+    launches0 = ctx.launch_count()
+    for _ in range(args.warmup):
+        copy_state(work, pristine)
+        ctx.source_update(work, dt, wl.c, wl.c_hat)
+    barrier()
+    launches0 = ctx.launch_count()
+    sampler = ClockSampler(local)
+    sampler.start()
+    evs = []
+    for _ in range(args.steps):
+        copy_state(work, pristine)           # untimed restore (also evicts the previous step from L2)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        ctx.source_update(work, dt, wl.c, wl.c_hat)
+        e1.record(stream)
+        evs.append((e0, e1))
+    barrier()
+    clocks = sampler.stop()
+    gpu_launches = ctx.launch_count() - launches0
+    step_ms = [a.elapsed_time(b) for a, b in evs]
+    total_ms = torch.tensor([sum(step_ms)], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(total_ms, op=dist.ReduceOp.MAX)
+    total_s = float(total_ms.item()) * 1e-3
+    value = world * n * Nq * args.steps / total_s
+    ms_per_step = 1e3 * total_s / args.steps
+
+    # ---- roofline (rank 0's kernel): ALU-bound; HBM figures alongside ----------------------------------
+    dfma = binding.measure_dfma_peak(1 << 22)              # FMA/s, measured now on this device
+    peak_tflops = 2.0 * dfma / 1e12
+    avg_launch_s = (sum(step_ms) / len(step_ms)) * 1e-3
+    achieved_tflops = flops_per_launch / avg_launch_s / 1e12
+    alg_bytes = 8.0 * n * ((5 + 4 * Nq) + (4 + 4 * Nq) + (0 if pristine["kappa_scale"] is None else 1))
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
+    roofline = {
+        "bound": "alu", "achieved": achieved_tflops, "peak": peak_tflops, "unit": "TFLOP/s",
+        "frac": achieved_tflops / peak_tflops, "traffic": NCU_TRAFFIC_BYTES.get(wl.index),
+        "peak_source": "FP64 FMA rate measured in this run by mgrhd_measure_dfma_peak (x2 flop/FMA)",
+        "algorithmic_flops_per_launch": flops_per_launch,
+        "algorithmic_flops_per_cell_group": flops_per_launch / (n * Nq),
+        "hbm": {"achieved_gbs": alg_bytes / avg_launch_s / 1e9, "peak_gbs": hbm_peak,
+                "frac": alg_bytes / avg_launch_s / 1e9 / hbm_peak, "algorithmic_bytes_per_launch": alg_bytes,
+                "peak_source": "MEASURED_PEAKS.json hbm_gbs" if peaks else "fallback 6650 GB/s"},
+    }
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_label(wl), "cells_per_gpu": n, "Nq": Nq, "dt": dt, "c": wl.c,
+                   "c_hat": wl.c_hat, "newton_tol": wl.newton_tol, "outer_stop": wl.outer_stop,
+                   "l2": "state (%.2f GB) larger than L2; restored from a pristine copy before every step"
+                         % (state_nbytes(pristine) / 1e9)},
+        "clocks": clocks, "gpu_launches": gpu_launches, "roofline": roofline,
+        "step_ms": step_ms,
+        "iterations": {"newton_evals_per_cell": stats["newton_evals_total"] / n,
+                       "outer_trips_per_cell": stats["outer_trips_total"] / n,
+                       "newton_evals_max": int(max(i for i, c in enumerate(stats["newton_hist"]) if c)),
+                       "outer_trips_max": int(max(i for i, c in enumerate(stats["outer_hist"]) if c)),
+                       "n_newton_unconverged": stats["n_newton_unconverged"],
+                       "n_outer_unconverged": stats["n_outer_unconverged"],
+                       "n_T_nonpositive_steps": stats["n_T_nonpositive_steps"],
+                       "n_chiF_guard": stats["n_chiF_guard"],
+                       "n_denominator_nonpositive": stats["n_denominator_nonpositive"]},
+        "conservation": {"energy_residual_max": resE, "momentum_residual_max": resP, "all_finite": finite},
+    }
+
+    # ---- end to end through the C ABI with HOST buffers (copies inside the timed region) ---------------
+    if not args.no_e2e:
+        line["e2e"] = run_e2e(args, wl, ctx, pristine, dt, world, dist if world > 1 else None)
+
+    # ---- CPU oracle beside it (rank 0, N = 1 only), with a parity check on the same cells --------------
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        line["cpu_baseline"], line["parity_sample"] = run_cpu_baseline(args, wl, pristine, work, dt)
+
+    ctx.free()
+    if rank == 0:
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the update kernel, from the
+# `ncu --set full` capture summarised under profiles/ (None until a capture of that workload exists).
+NCU_TRAFFIC_BYTES: dict = {}
+
+
+def run_e2e(args, wl, ctx, pristine, dt, world, dist):
+    """The same metric through mgrhd_source_update_host: pinned HOST buffers in, HOST buffers out,
+    every host<->device copy inside the timed region.  Falls back to fewer cells if the host cannot
+    pin the whole state."""
+    import torch
+
+    n, Nq = wl.ncells, wl.Nq
+    cells = n
+    host = None
+    while host is None:
+        try:
+            sub = {k: (None if v is None else v[..., :cells]) for k, v in pristine.items()}
+            host = alloc_like(sub, pin=True)
+        except RuntimeError:
+            host = None
+            cells //= 4
+            if cells < 1024:
+                return {"value": None, "unit": UNIT, "error": "could not allocate pinned host buffers"}
+    sub = {k: (None if v is None else v[..., :cells]) for k, v in pristine.items()}
+    times = []
+    for step in range(1 + args.e2e_steps):
+        copy_state(host, sub)                       # untimed: put U^(t) into the host buffers
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        t0 = time.perf_counter()
+        ctx.source_update_host(host, dt, wl.c, wl.c_hat)   # synchronous: returns with U^(t+1) on the host
+        t1 = time.perf_counter()
+        if step >= 1:
+            times.append(t1 - t0)
+    t = torch.tensor([sum(times)], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total = float(t.item())
+    h2d = state_nbytes(host)
+    d2h = state_nbytes(host, keys=("mom", "Egas", "Erad", "Frad"))
+    return {"value": world * cells * Nq * len(times) / total, "unit": UNIT, "h2d_bytes_per_step": h2d,
+            "d2h_bytes_per_step": d2h, "cells_per_gpu": cells, "steps": len(times),
+            "ms_per_step": 1e3 * total / len(times), "timer": "host wall clock around the synchronous C-ABI call",
+            "host_memory": "pinned"}
+
+
+def run_cpu_baseline(args, wl, pristine, work, dt):
+    """Oracle on the first M cells (one host core), and parity of the GPU result on the same cells."""
+    import numpy as np
+    import torch
+
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    from parity_util import compare
+
+    from paper_2407_18304_b200 import workloads as W
+
+    M = min(wl.ncells, args.cpu_sample_cells or default_cpu_sample(wl))
+    st0 = W.to_numpy({k: (None if v is None else v[..., :M]) for k, v in pristine.items()})
+    ref = {k: (None if v is None else v.copy()) for k, v in st0.items()}
+    secs, ost = time_oracle(wl, ref, dt)
+    got = W.to_numpy({k: (None if v is None else v[..., :M]) for k, v in work.items()})   # last timed step's result
+    res = compare(ref, got, st0, wl.c, wl.c_hat)
+    cpu = {"value": M * wl.Nq / secs, "unit": UNIT, "cores": 1, "kind": "oracle",
+           "sample": f"first {M} cells of {workload_label(wl)}, one update, single thread, dense LU", "seconds": secs,
+           "host_cores_available": os.cpu_count()}
+    parity = {"cells": M, "tolerance": "|d| <= 1e-10|ref| + 1e-14 S_cell", "ok": all(v[0] == 0 for v in res.values()),
+              "worst_excess_ratio": {k: v[1] for k, v in res.items()},
+              "oracle_newton_evals_per_cell": ost["newton_evals_total"] / M}
+    return cpu, parity
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

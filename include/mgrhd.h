@@ -84,6 +84,7 @@ typedef struct {
   long long n_denominator_nonpositive; /* cell-groups with 1 + c_hat chi_F dt <= 0              */
   long long newton_evals_total;        /* residual evaluations (Eq. 41), summed over cells      */
   long long outer_trips_total;         /* outer trips, summed over cells                        */
+  long long flops;                     /* algorithmic FP64 flops (0 unless counting is on)      */
   long long newton_hist[MGRHD_HIST];   /* per-cell residual evaluations (clamped)               */
   long long outer_hist[MGRHD_HIST];    /* per-cell outer trips (clamped)                        */
 } mgrhd_stats;
@@ -123,6 +124,10 @@ int mgrhd_conserved_totals(mgrhd_ctx *ctx, const mgrhd_state *state_dev, long lo
 int mgrhd_get_stats(mgrhd_ctx *ctx, mgrhd_stats *host_out);
 /* Zero the device counters (stream-ordered on the last stream used). */
 int mgrhd_reset_stats(mgrhd_ctx *ctx);
+/* Switch the instrumented kernels on (1) or off (0, default): they also accumulate the
+ * ALGORITHMIC FP64 flop count of the update (FMA = 2) into
+ * mgrhd_stats.flops.  Used by bench.py for the ALU roofline; never on in a timed region. */
+int mgrhd_set_flop_counting(mgrhd_ctx *ctx, int on);
 /* Number of kernels this context has launched so far (for bench.py's gpu_launches). */
 long long mgrhd_launch_count(const mgrhd_ctx *ctx);
 

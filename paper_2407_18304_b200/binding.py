@@ -19,7 +19,7 @@ HIST = 64
 
 EXPORTS = (
     "mgrhd_init", "mgrhd_source_update", "mgrhd_source_update_host", "mgrhd_conserved_totals",
-    "mgrhd_get_stats", "mgrhd_reset_stats", "mgrhd_launch_count", "mgrhd_measure_dfma_peak",
+    "mgrhd_get_stats", "mgrhd_reset_stats", "mgrhd_set_flop_counting", "mgrhd_launch_count", "mgrhd_measure_dfma_peak",
     "mgrhd_last_error", "mgrhd_free",
 )
 
@@ -46,7 +46,7 @@ class Stats(ctypes.Structure):
     _fields_ = [("n_cells", ctypes.c_longlong), ("n_newton_unconverged", ctypes.c_longlong),
                 ("n_outer_unconverged", ctypes.c_longlong), ("n_T_nonpositive_steps", ctypes.c_longlong),
                 ("n_chiF_guard", ctypes.c_longlong), ("n_denominator_nonpositive", ctypes.c_longlong),
-                ("newton_evals_total", ctypes.c_longlong), ("outer_trips_total", ctypes.c_longlong),
+                ("newton_evals_total", ctypes.c_longlong), ("outer_trips_total", ctypes.c_longlong), ("flops", ctypes.c_longlong),
                 ("newton_hist", ctypes.c_longlong * HIST), ("outer_hist", ctypes.c_longlong * HIST)]
 
 
@@ -79,6 +79,8 @@ def load_library() -> ctypes.CDLL:
     L.mgrhd_get_stats.argtypes = [vp, ctypes.POINTER(Stats)]
     L.mgrhd_reset_stats.restype = i
     L.mgrhd_reset_stats.argtypes = [vp]
+    L.mgrhd_set_flop_counting.restype = i
+    L.mgrhd_set_flop_counting.argtypes = [vp, i]
     L.mgrhd_launch_count.restype = ll
     L.mgrhd_launch_count.argtypes = [vp]
     L.mgrhd_measure_dfma_peak.restype = i
@@ -197,6 +199,9 @@ class Context:
 
     def reset_stats(self) -> None:
         _check(self._L.mgrhd_reset_stats(self._h), "mgrhd_reset_stats")
+
+    def set_flop_counting(self, on: bool) -> None:
+        _check(self._L.mgrhd_set_flop_counting(self._h, 1 if on else 0), "mgrhd_set_flop_counting")
 
     def launch_count(self) -> int:
         return int(self._L.mgrhd_launch_count(self._h))

@@ -83,6 +83,7 @@ struct mgrhd_ctx {
   unsigned long long* d_stats;
   cudaStream_t last_stream;
   long long launches;
+  int count_flops;
   // host-buffer path scratch (lazily allocated)
   double* slab[kSlabs];
   long long slab_cells;
@@ -172,11 +173,17 @@ static int launch_update(mgrhd_ctx* ctx, const StatePtrs& S, long long n, long l
   const long long cap = (long long)ctx->sm_count * 64;
   if (blocks > cap) blocks = cap;
   const dim3 grid((unsigned)blocks), block(kBlock);
-  if (P.Nq <= 4) source_update_kernel<4><<<grid, block, 0, st>>>(P, S, ctx->d_stats);
-  else if (P.Nq <= 8) source_update_kernel<8><<<grid, block, 0, st>>>(P, S, ctx->d_stats);
-  else if (P.Nq <= 16) source_update_kernel<16><<<grid, block, 0, st>>>(P, S, ctx->d_stats);
-  else if (P.Nq <= 32) source_update_kernel<32><<<grid, block, 0, st>>>(P, S, ctx->d_stats);
-  else source_update_kernel<64><<<grid, block, 0, st>>>(P, S, ctx->d_stats);
+#define MGRHD_LAUNCH(Q)                                                                  \
+  do {                                                                                   \
+    if (ctx->count_flops) source_update_kernel<Q, true><<<grid, block, 0, st>>>(P, S, ctx->d_stats);   \
+    else source_update_kernel<Q, false><<<grid, block, 0, st>>>(P, S, ctx->d_stats);     \
+  } while (0)
+  if (P.Nq <= 4) MGRHD_LAUNCH(4);
+  else if (P.Nq <= 8) MGRHD_LAUNCH(8);
+  else if (P.Nq <= 16) MGRHD_LAUNCH(16);
+  else if (P.Nq <= 32) MGRHD_LAUNCH(32);
+  else MGRHD_LAUNCH(64);
+#undef MGRHD_LAUNCH
   ctx->launches++;
   ctx->last_stream = st;
   CU(cudaGetLastError());
@@ -288,6 +295,7 @@ int mgrhd_get_stats(mgrhd_ctx* ctx, mgrhd_stats* out) {
   out->n_denominator_nonpositive = (long long)h[kStatDenNonPos];
   out->newton_evals_total = (long long)h[kStatNewtonEvals];
   out->outer_trips_total = (long long)h[kStatOuterTrips];
+  out->flops = (long long)h[kStatFlops];
   for (int b = 0; b < MGRHD_HIST; ++b) {
     out->newton_hist[b] = (long long)h[kStatNewtonHist + b];
     out->outer_hist[b] = (long long)h[kStatOuterHist + b];
@@ -298,6 +306,12 @@ int mgrhd_get_stats(mgrhd_ctx* ctx, mgrhd_stats* out) {
 int mgrhd_reset_stats(mgrhd_ctx* ctx) {
   if (!ctx) return MGRHD_ERR_ARG;
   CU(cudaMemsetAsync(ctx->d_stats, 0, kStatCount * sizeof(unsigned long long), ctx->last_stream));
+  return MGRHD_OK;
+}
+
+int mgrhd_set_flop_counting(mgrhd_ctx* ctx, int on) {
+  if (!ctx) return MGRHD_ERR_ARG;
+  ctx->count_flops = on ? 1 : 0;
   return MGRHD_OK;
 }
 

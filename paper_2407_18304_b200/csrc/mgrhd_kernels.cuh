@@ -40,7 +40,7 @@ __device__ __forceinline__ void closure_vP(int closure, double E, double F0, dou
 }
 
 // MAXQ: compile-time bound on Nq (per-thread group arrays are sized MAXQ).
-template <int MAXQ>
+template <int MAXQ, bool COUNT>
 __global__ void __launch_bounds__(128)
 source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ StatePtrs S,
                      unsigned long long* __restrict__ stats) {
@@ -55,6 +55,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
 
   unsigned int cnt_newton_unconv = 0, cnt_outer_unconv = 0, cnt_Tnonpos = 0, cnt_guard = 0,
                cnt_den = 0, cnt_evals = 0, cnt_trips = 0, cnt_cells = 0;
+  unsigned long long flops = 0;
 
   for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n;
        i += (long long)gridDim.x * blockDim.x) {
@@ -83,6 +84,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
       sumEt += Et[g];
     }
     const double Etot = Egas_t + (chat / c) * sumEt;   // Eq. 50 as printed, S_g = 0
+    if (COUNT) flops += kFlopCell + kFlopCellGroup * Nq;
 
     double momk0 = momt0, momk1 = momt1, momk2 = momt2;
     double momn0 = momt0, momn1 = momt1, momn2 = momt2;
@@ -109,11 +111,13 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
         const double beta = P.h_over_k / T;
         double sumR = 0.0, sumAbsFR = 0.0, S1 = 0.0, S2 = 0.0;
         EdgeFn lo = planck_edge(P.nu[0] * beta);
+        if (COUNT) flops += kFlopCellEval + lo.flops + (unsigned)(kFlopGroupEval * Nq);
         if (P.nu[0] == 0.0) { lo.yz = 0.0; lo.xi = 0.0; lo.small = true; }
         for (int g = 0; g < Nq; ++g) {
           // a1: edge functions at the upper edge of group g
           const double nuh = P.nu[g + 1];
           EdgeFn hi = planck_edge(nuh * beta);
+          if (COUNT) flops += hi.flops;
           // a2: group Planck integral and Doppler boundary terms (Eq. 11, 18, 22)
           const double chi_lo = chis * P.k_lo[g], chi_hi = chis * P.k_hi[g];
           const double chiE = chis * P.k_mean[g];            // = chi_B (alpha_Q = -1 for both)
@@ -167,6 +171,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
           cnt_Tnonpos++;
         }
         Egs += lam * dx0;
+        if (COUNT) flops += kFlopStepCell + kFlopStepGroup * Nq;
         for (int g = 0; g < Nq; ++g) R[g] += lam * (da[g] + db[g] * dx0);
       }
 
@@ -201,6 +206,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
       const double icc = 1.0 / (c * chat);
       momn0 = momt0 - dF0 * icc; momn1 = momt1 - dF1 * icc; momn2 = momt2 - dF2 * icc;
       trips++;
+      if (COUNT) flops += kFlopOuterCell + kFlopOuterGroup * Nq;
 
       // ---- a9: outer convergence (reading S10) ------------------------
       const double vn0 = momn0 / rho, vn1 = momn1 / rho, vn2 = momn2 / rho;
@@ -249,6 +255,10 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
     unsigned int v = vals[s];
     for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
     if ((threadIdx.x & 31) == 0 && v) atomicAdd(&stats[s], (unsigned long long)v);
+  }
+  if (COUNT) {
+    for (int off = 16; off > 0; off >>= 1) flops += __shfl_xor_sync(0xffffffffu, flops, off);
+    if ((threadIdx.x & 31) == 0) atomicAdd(&stats[kStatFlops], flops);
   }
   __syncthreads();
   for (int t = threadIdx.x; t < 2 * MGRHD_HIST; t += blockDim.x)

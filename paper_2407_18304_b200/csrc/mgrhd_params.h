@@ -24,10 +24,28 @@ enum StatSlot {
   kStatDenNonPos,
   kStatNewtonEvals,
   kStatOuterTrips,
+  kStatFlops,                            // algorithmic FP64 flops (counting launches only)
   kStatNewtonHist,                       // MGRHD_HIST slots
   kStatOuterHist = kStatNewtonHist + MGRHD_HIST,
   kStatCount = kStatOuterHist + MGRHD_HIST
 };
+
+// Algorithmic FP64 flop counts of each piece of the update as written in mgrhd_kernels.cuh
+// (FMA = 2; add, mul, div, sqrt = 1; exp = kFlopExp; comparisons, fabs, selects = 0).
+// Derived line by line in DESIGN.md "Algorithmic flops"; used only by the counting kernels.
+constexpr int kFlopExp = 30;          // range reduction + degree-11 polynomial + scaling
+constexpr int kFlopEdgeSmall = 75;    // x < kXSplit: two 16-term Horner chains + assembly
+constexpr int kFlopEdgeLargeBase = 42;  // x >= kXSplit: exp, powers, Xi with one division
+constexpr int kFlopEdgeTerm = 11;     // one term of the e^{-nx} series
+constexpr int kFlopEdgeZero = 32;     // e^{-x} underflowed
+constexpr int kFlopGroupEval = 62;    // a2-a5 for one group at one trial T
+constexpr int kFlopCellEval = 13;     // T, a_R T^4, beta, F_G, Eq. 49
+constexpr int kFlopStepCell = 9;      // dx0, T>0 check, E_gas update
+constexpr int kFlopStepGroup = 4;     // R_g += lam (da + db dx0)
+constexpr int kFlopOuterCell = 45;    // v, E_kin, commit, Eq. 52, outer test
+constexpr int kFlopOuterGroup = 106;  // closure, Eq. 51, relative-change test, next v.F_g, dW
+constexpr int kFlopCell = 6;          // load-time derivations
+constexpr int kFlopCellGroup = 7;     // sum E_g, first v.F_g, E_g commit
 
 struct Params {
   // ---- group structure and opacity table (set once by mgrhd_init) -------------------

@@ -24,6 +24,7 @@ struct EdgeFn {
   double yz;   // Y(x) if small, else Z(x)
   double xi;   // Xi(x)
   bool small;  // which of the two yz holds
+  int flops;   // algorithmic flop count of this evaluation (dead code unless counted)
 };
 
 // x in [0, +inf].  x == 0 -> (Y=0, Xi=0); x == +inf or e^-x == 0 -> (Z=0, Xi=0).
@@ -43,6 +44,7 @@ __device__ __forceinline__ EdgeFn planck_edge(double x) {
     r.yz = kC15Pi4 * x3 * fma(x2, sy, fma(-0.125, x, 1.0 / 3.0));
     r.xi = kC15Pi4 * x3 * fma(x2, sx, fma(-0.5, x, 1.0));
     r.small = true;
+    r.flops = kFlopEdgeSmall;
     return r;
   }
   r.small = false;
@@ -50,23 +52,27 @@ __device__ __forceinline__ EdgeFn planck_edge(double x) {
   if (!(u > 0.0)) {  // underflow or x = +inf
     r.yz = 0.0;
     r.xi = 0.0;
+    r.flops = kFlopEdgeZero;
     return r;
   }
   const double x2 = x * x, x3 = x2 * x;
   const double c3 = x3, c2 = 3.0 * x2, c1 = 6.0 * x, c0 = 6.0;
   double un = u;     // u^n
   double sum = 0.0;
+  int nt = 0;
   for (int n = 1; n <= kSeriesMax; ++n) {
     const double q = c_planck.inv_n[n];
     // x^3/n + 3x^2/n^2 + 6x/n^3 + 6/n^4  by Horner in 1/n
     const double pn = q * fma(q, fma(q, fma(q, c0, c1), c2), c3);
     const double term = un * pn;
     sum += term;
+    ++nt;
     if (term <= 1e-18 * sum) break;
     un *= u;
   }
   r.yz = kC15Pi4 * sum;
   r.xi = kC15Pi4 * (x2 * x2) * (u / (1.0 - u));
+  r.flops = kFlopEdgeLargeBase + kFlopEdgeTerm * nt;
   return r;
 }
 

@@ -41,7 +41,7 @@ def test_struct_layouts_match_header(binding):
     """ctypes mirrors: field counts/sizes implied by the header."""
     assert ctypes.sizeof(binding.Units) == 5 * 8
     assert ctypes.sizeof(binding.State) == 10 * 8
-    assert ctypes.sizeof(binding.Stats) == (8 + 2 * 64) * 8
+    assert ctypes.sizeof(binding.Stats) == (9 + 2 * 64) * 8
     src = open(HEADER).read()
     assert "#define MGRHD_MAX_GROUPS 64" in src and "#define MGRHD_HIST 64" in src
     assert binding.MAX_GROUPS == 64 and binding.HIST == 64
