@@ -131,6 +131,12 @@ int mgrhd_set_flop_counting(mgrhd_ctx *ctx, int on);
 /* Number of kernels this context has launched so far (for bench.py's gpu_launches). */
 long long mgrhd_launch_count(const mgrhd_ctx *ctx);
 
+/* Diagnostic: the kernel's Planck edge functions on n DEVICE values x >= 0 (x = h nu/(k_B T)):
+ *   is_y[i] = 1: yz[i] = Y(x) = (15/pi^4) int_0^x t^3/(e^t-1) dt;  is_y[i] = 0: yz[i] = 1 - Y(x);
+ *   xi[i] = (15/pi^4) x^4/(e^x-1).  (Eq. 11 applied to B_nu.)  Stream-ordered. */
+int mgrhd_planck_edge_functions(const double *x_dev, long long n, double *yz_dev, double *xi_dev,
+                                int *is_y_dev, void *cuda_stream);
+
 /* Sustained FP64 FMA rate of the current device in FMA/s (a dependent-chain-free DFMA
  * microbenchmark, `iters` FMAs per thread; used as the ALU roofline denominator). */
 int mgrhd_measure_dfma_peak(long long iters, double *fma_per_second);

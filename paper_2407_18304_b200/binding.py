@@ -19,7 +19,7 @@ HIST = 64
 
 EXPORTS = (
     "mgrhd_init", "mgrhd_source_update", "mgrhd_source_update_host", "mgrhd_conserved_totals",
-    "mgrhd_get_stats", "mgrhd_reset_stats", "mgrhd_set_flop_counting", "mgrhd_launch_count", "mgrhd_measure_dfma_peak",
+    "mgrhd_get_stats", "mgrhd_reset_stats", "mgrhd_set_flop_counting", "mgrhd_launch_count", "mgrhd_planck_edge_functions", "mgrhd_measure_dfma_peak",
     "mgrhd_last_error", "mgrhd_free",
 )
 
@@ -83,6 +83,8 @@ def load_library() -> ctypes.CDLL:
     L.mgrhd_set_flop_counting.argtypes = [vp, i]
     L.mgrhd_launch_count.restype = ll
     L.mgrhd_launch_count.argtypes = [vp]
+    L.mgrhd_planck_edge_functions.restype = i
+    L.mgrhd_planck_edge_functions.argtypes = [vp, ll, vp, vp, vp, vp]
     L.mgrhd_measure_dfma_peak.restype = i
     L.mgrhd_measure_dfma_peak.argtypes = [ll, _dp]
     L.mgrhd_last_error.restype = ctypes.c_char_p
@@ -223,3 +225,16 @@ def measure_dfma_peak(iters: int = 1 << 20) -> float:
     out = ctypes.c_double(0.0)
     _check(load_library().mgrhd_measure_dfma_peak(iters, ctypes.byref(out)), "mgrhd_measure_dfma_peak")
     return out.value
+
+
+def planck_edge_functions(x):
+    """mgrhd_planck_edge_functions on a CUDA float64 tensor x; returns (yz, xi, is_y) tensors."""
+    import torch
+
+    assert x.is_cuda and x.dtype == torch.float64 and x.is_contiguous()
+    yz, xi = torch.empty_like(x), torch.empty_like(x)
+    is_y = torch.empty(x.shape, dtype=torch.int32, device=x.device)
+    _check(load_library().mgrhd_planck_edge_functions(x.data_ptr(), x.numel(), yz.data_ptr(), xi.data_ptr(),
+                                                      is_y.data_ptr(), ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)),
+           "mgrhd_planck_edge_functions")
+    return yz, xi, is_y

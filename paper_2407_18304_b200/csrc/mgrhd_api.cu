@@ -6,6 +6,7 @@
 
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <mutex>
 #include <new>
@@ -42,16 +43,71 @@ long double zeta_even(int n) {
 
 // b_{2n} = B_{2n}/(2n)! = (-1)^(n+1) 2 zeta(2n)/(2 pi)^(2n): Maclaurin coefficients of
 // t/(e^t-1) = 1 - t/2 + sum_n b_{2n} t^(2n).
-void fill_planck_tables(PlanckTables& t) {
+long double bern_over_fact(int n) {
   const long double TWO_PI = 6.28318530717958647692528676655900577L;
+  long double b = 2.0L * zeta_even(n) / powl(TWO_PI, 2.0L * n);
+  return (n % 2 == 0) ? -b : b;
+}
+
+const long double kC15Pi4L = 15.0L / (3.14159265358979323846264338327950288L * 3.14159265358979323846264338327950288L *
+                                      3.14159265358979323846264338327950288L * 3.14159265358979323846264338327950288L);
+
+// Reference values for the mid-range fits, long double, x >= 1:
+//   Z(x) = C sum_n e^{-nx}(x^3/n + 3x^2/n^2 + 6x/n^3 + 6/n^4),  Xi(x) = C x^4/(e^x - 1).
+long double Z_host(long double x) {
+  long double sum = 0.0L;
+  for (int n = 1; n <= 200; ++n) {
+    const long double q = 1.0L / n;
+    const long double term = expl(-n * x) * q * (x * x * x + q * (3.0L * x * x + q * (6.0L * x + q * 6.0L)));
+    sum += term;
+    if (term < 1e-24L * sum) break;
+  }
+  return kC15Pi4L * sum;
+}
+long double Xi_host(long double x) { return kC15Pi4L * x * x * x * x / expm1l(x); }
+
+// Chebyshev interpolation of f on [a,b] with N nodes, truncated to M terms and rewritten as a
+// monomial series in t = (2x - a - b)/(b - a): out[k] t^k.
+void cheb_fit_monomial(long double (*f)(long double), long double a, long double b, int N, int M, double* out) {
+  const long double PI = 3.14159265358979323846264338327950288L;
+  long double fx[64], ck[64], mono[64] = {0}, Tkm1[64] = {0}, Tk[64] = {0}, Tn[64];
+  for (int j = 0; j < N; ++j) fx[j] = f(0.5L * (a + b) + 0.5L * (b - a) * cosl(PI * (j + 0.5L) / N));
+  for (int k = 0; k < M; ++k) {
+    long double s = 0.0L;
+    for (int j = 0; j < N; ++j) s += fx[j] * cosl(PI * k * (j + 0.5L) / N);
+    ck[k] = 2.0L * s / N;
+  }
+  ck[0] *= 0.5L;
+  // T_0 = 1, T_1 = t, T_{k+1} = 2 t T_k - T_{k-1}, as monomial coefficient vectors
+  Tkm1[0] = 1.0L;
+  Tk[1] = 1.0L;
+  mono[0] += ck[0];
+  if (M > 1) mono[1] += ck[1];
+  for (int k = 2; k < M; ++k) {
+    for (int i = 0; i < 64; ++i) Tn[i] = -Tkm1[i];
+    for (int i = 0; i + 1 < 64; ++i) Tn[i + 1] += 2.0L * Tk[i];
+    for (int i = 0; i < 64; ++i) { mono[i] += ck[k] * Tn[i]; Tkm1[i] = Tk[i]; Tk[i] = Tn[i]; }
+  }
+  for (int k = 0; k < M; ++k) out[k] = (double)mono[k];
+}
+
+void fill_planck_tables(PlanckTables& t) {
   for (int n = 1; n <= kSmallTerms; ++n) {
-    long double b = 2.0L * zeta_even(n) / powl(TWO_PI, 2.0L * n);
-    if (n % 2 == 0) b = -b;
+    const long double b = bern_over_fact(n);
     t.xi_c[n - 1] = (double)b;
     t.y_c[n - 1] = (double)(b / (2.0L * n + 3.0L));
   }
-  t.inv_n[0] = 0.0;
-  for (int n = 1; n <= kSeriesMax; ++n) t.inv_n[n] = (double)(1.0L / (long double)n);
+  cheb_fit_monomial(Z_host, kXS, kXL, 48, kMidTerms, t.mz);
+  cheb_fit_monomial(Xi_host, kXS, kXL, 48, kMidTerms, t.mx);
+  t.mid_s = (double)(2.0L / ((long double)kXL - (long double)kXS));
+  t.mid_o = (double)(-((long double)kXL + (long double)kXS) / ((long double)kXL - (long double)kXS));
+  for (int n = 1; n <= kLargeTerms; ++n) {
+    const long double q = 1.0L / n;
+    t.l3[n - 1] = (double)(kC15Pi4L * q);
+    t.l2[n - 1] = (double)(3.0L * kC15Pi4L * q * q);
+    t.l1[n - 1] = (double)(6.0L * kC15Pi4L * q * q * q);
+    t.l0[n - 1] = (double)(6.0L * kC15Pi4L * q * q * q * q);
+  }
 }
 
 std::once_flag g_tables_once[16];  // per device
@@ -70,7 +126,6 @@ cudaError_t upload_tables_for_current_device() {
   return g_tables_err[dev];
 }
 
-constexpr int kBlock = 128;
 constexpr int kSlabs = 3;                       // host path: slabs in flight
 constexpr long long kSlabBytes = 96ll << 20;    // target bytes per slab
 
@@ -84,11 +139,70 @@ struct mgrhd_ctx {
   cudaStream_t last_stream;
   long long launches;
   int count_flops;
+  int variant, cfg_nsmem;
+  int cfg_nq, cfg_threads, cfg_bps;   // kernel instantiation, CTA size, resident CTAs per SM
+  double* scratch;                    // lagged-flux scratch of the device path
+  double* slab_scratch[kSlabs];       // ... and of each host-path slab stream
   // host-buffer path scratch (lazily allocated)
   double* slab[kSlabs];
   long long slab_cells;
   cudaStream_t slab_stream[kSlabs];
 };
+
+// One instantiation per group capacity: CTA size chosen so the [slot][group][thread] state fits
+// in shared memory (SL_COUNT * NQ * THREADS * 8 bytes <= 192 KB).
+template <int NQ, int THREADS, int NSMEM>
+struct Inst {
+  static constexpr size_t kSmem = (size_t)NSMEM * NQ * THREADS * sizeof(double);
+  static cudaError_t configure(int* blocks_per_sm) {
+    cudaError_t e = cudaFuncSetAttribute(source_update_kernel<NQ, THREADS, NSMEM, false>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem);
+    if (e == cudaSuccess)
+      e = cudaFuncSetAttribute(source_update_kernel<NQ, THREADS, NSMEM, true>,
+                               cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem);
+    if (e == cudaSuccess)
+      e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, source_update_kernel<NQ, THREADS, NSMEM, false>,
+                                                        THREADS, kSmem);
+    return e;
+  }
+  static void launch(bool count, unsigned blocks, cudaStream_t st, const Params& P, const StatePtrs& S,
+                     unsigned long long* stats, double* scratch) {
+    if (count) source_update_kernel<NQ, THREADS, NSMEM, true><<<blocks, THREADS, kSmem, st>>>(P, S, stats, scratch);
+    else source_update_kernel<NQ, THREADS, NSMEM, false><<<blocks, THREADS, kSmem, st>>>(P, S, stats, scratch);
+  }
+};
+
+#define MGRHD_DISPATCH(Nq, V, WHAT)                            \
+  do {                                                         \
+    if ((Nq) <= 4) { WHAT(4, 256, 6); }                        \
+    else if ((Nq) <= 8) { WHAT(8, 256, 6); }                   \
+    else if ((Nq) <= 16) { WHAT(16, 256, 6); }                 \
+    else if ((Nq) <= 32) {                                     \
+      if ((V) == 1) { WHAT(32, 192, 4); }                      \
+      else if ((V) == 2) { WHAT(32, 256, 3); }                 \
+      else if ((V) == 3) { WHAT(32, 384, 2); }                 \
+      else if ((V) == 4) { WHAT(32, 512, 0); }                 \
+      else { WHAT(32, 128, 6); }                               \
+    }                                                          \
+    else { WHAT(64, 64, 6); }                                  \
+  } while (0)
+
+// Fills ctx->cfg_* for ctx->P.Nq (called once by mgrhd_init).
+static cudaError_t configure_ctx(mgrhd_ctx* ctx) {
+  cudaError_t e = cudaSuccess;
+  const char* ev = getenv("MGRHD_VARIANT");
+  ctx->variant = ev ? atoi(ev) : 0;
+#define MGRHD_CFG(Q, T, M) e = Inst<Q, T, M>::configure(&ctx->cfg_bps); ctx->cfg_nq = Q; ctx->cfg_threads = T; ctx->cfg_nsmem = M
+  MGRHD_DISPATCH(ctx->P.Nq, ctx->variant, MGRHD_CFG);
+#undef MGRHD_CFG
+  if (e == cudaSuccess && ctx->cfg_bps < 1) e = cudaErrorLaunchOutOfResources;
+  return e;
+}
+
+// Bytes of lagged-flux scratch one launch needs at most: 3 * NQ doubles per resident thread.
+static size_t scratch_bytes(const mgrhd_ctx* ctx) {
+  return (size_t)(3 + SL_COUNT - ctx->cfg_nsmem) * ctx->cfg_nq * sizeof(double) * (size_t)ctx->sm_count * ctx->cfg_bps * ctx->cfg_threads;
+}
 
 extern "C" {
 
@@ -139,15 +253,20 @@ int mgrhd_init(mgrhd_ctx** out, const double* edges, int Nq, const mgrhd_units* 
       P.k_mean[g] = k * (std::expm1(z) / z);
     }
     P.inv_k_mean[g] = 1.0 / P.k_mean[g];
+    P.k_num[g] = P.k_mean[g] * ((4.0 + a) / 3.0);
+    P.onepa[g] = 1.0 + a;
   }
   cudaError_t e = cudaGetDevice(&ctx->device);
   if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, ctx->device);
   if (e == cudaSuccess) e = upload_tables_for_current_device();
+  if (e == cudaSuccess) e = configure_ctx(ctx);
+  if (e == cudaSuccess) e = cudaMalloc(&ctx->scratch, scratch_bytes(ctx));
   if (e == cudaSuccess) e = cudaMalloc(&ctx->d_stats, kStatCount * sizeof(unsigned long long));
   if (e == cudaSuccess) e = cudaMemset(ctx->d_stats, 0, kStatCount * sizeof(unsigned long long));
   if (e != cudaSuccess) {
     cuda_ok(e, "mgrhd_init");
     if (ctx->d_stats) cudaFree(ctx->d_stats);
+    if (ctx->scratch) cudaFree(ctx->scratch);
     delete ctx;
     return MGRHD_ERR_CUDA;
   }
@@ -166,24 +285,17 @@ static int check_call(const mgrhd_ctx* ctx, const mgrhd_state* s, long long n, d
 }
 
 static int launch_update(mgrhd_ctx* ctx, const StatePtrs& S, long long n, long long stride, double dt,
-                         double c, double chat, cudaStream_t st) {
+                         double c, double chat, cudaStream_t st, double* scratch) {
   Params P = ctx->P;
   P.dt = dt; P.c = c; P.c_hat = chat; P.ncells = n; P.stride = stride;
-  long long blocks = (n + kBlock - 1) / kBlock;
-  const long long cap = (long long)ctx->sm_count * 64;
-  if (blocks > cap) blocks = cap;
-  const dim3 grid((unsigned)blocks), block(kBlock);
-#define MGRHD_LAUNCH(Q)                                                                  \
-  do {                                                                                   \
-    if (ctx->count_flops) source_update_kernel<Q, true><<<grid, block, 0, st>>>(P, S, ctx->d_stats);   \
-    else source_update_kernel<Q, false><<<grid, block, 0, st>>>(P, S, ctx->d_stats);     \
-  } while (0)
-  if (P.Nq <= 4) MGRHD_LAUNCH(4);
-  else if (P.Nq <= 8) MGRHD_LAUNCH(8);
-  else if (P.Nq <= 16) MGRHD_LAUNCH(16);
-  else if (P.Nq <= 32) MGRHD_LAUNCH(32);
-  else MGRHD_LAUNCH(64);
-#undef MGRHD_LAUNCH
+  // persistent grid: one CTA per resident slot, fewer when the problem is small
+  long long blocks = (long long)ctx->sm_count * ctx->cfg_bps;
+  const long long want = (n + ctx->cfg_threads - 1) / ctx->cfg_threads;
+  if (blocks > want) blocks = want;
+  const bool count = ctx->count_flops != 0;
+#define MGRHD_GO(Q, T, M) Inst<Q, T, M>::launch(count, (unsigned)blocks, st, P, S, ctx->d_stats, scratch)
+  MGRHD_DISPATCH(P.Nq, ctx->variant, MGRHD_GO);
+#undef MGRHD_GO
   ctx->launches++;
   ctx->last_stream = st;
   CU(cudaGetLastError());
@@ -205,7 +317,7 @@ int mgrhd_source_update(mgrhd_ctx* ctx, const mgrhd_state* s, long long n, doubl
   int rc = check_call(ctx, s, n, dt, c, chat);
   if (rc != MGRHD_OK) return rc;
   if (n == 0) return MGRHD_OK;
-  return launch_update(ctx, to_ptrs(s), n, n, dt, c, chat, (cudaStream_t)stream);
+  return launch_update(ctx, to_ptrs(s), n, n, dt, c, chat, (cudaStream_t)stream, ctx->scratch);
 }
 
 int mgrhd_conserved_totals(mgrhd_ctx* ctx, const mgrhd_state* s, long long n, double c, double chat,
@@ -238,6 +350,7 @@ int mgrhd_source_update_host(mgrhd_ctx* ctx, const mgrhd_state* s, long long n, 
     if (sc < 1024) sc = 1024;
     for (int j = 0; j < kSlabs; ++j) {
       CU(cudaMalloc(&ctx->slab[j], (size_t)sc * per_cell * sizeof(double)));
+      CU(cudaMalloc(&ctx->slab_scratch[j], scratch_bytes(ctx)));
       CU(cudaStreamCreateWithFlags(&ctx->slab_stream[j], cudaStreamNonBlocking));
     }
     ctx->slab_cells = sc;
@@ -268,7 +381,7 @@ int mgrhd_source_update_host(mgrhd_ctx* ctx, const mgrhd_state* s, long long n, 
     for (int i = 0; i < 3; ++i)
       CU(cudaMemcpy2DAsync(S.Frad[i], pitch_d, s->Frad[i] + lo, pitch_h, w, Nq, cudaMemcpyHostToDevice, st));
     // update
-    rc = launch_update(ctx, S, m, sc, dt, c, chat, st);
+    rc = launch_update(ctx, S, m, sc, dt, c, chat, st, ctx->slab_scratch[j]);
     if (rc != MGRHD_OK) return rc;
     // device -> host (rho and kappa_scale are read only)
     for (int i = 0; i < 3; ++i) CU(cudaMemcpyAsync(s->mom[i] + lo, S.mom[i], w, cudaMemcpyDeviceToHost, st));
@@ -317,6 +430,18 @@ int mgrhd_set_flop_counting(mgrhd_ctx* ctx, int on) {
 
 long long mgrhd_launch_count(const mgrhd_ctx* ctx) { return ctx ? ctx->launches : 0; }
 
+int mgrhd_planck_edge_functions(const double* x_dev, long long n, double* yz_dev, double* xi_dev,
+                                int* is_y_dev, void* stream) {
+  if (n < 0 || (n > 0 && (!x_dev || !yz_dev || !xi_dev || !is_y_dev))) return MGRHD_ERR_ARG;
+  if (n == 0) return MGRHD_OK;
+  CU(upload_tables_for_current_device());
+  long long blocks = (n + 255) / 256;
+  if (blocks > 4096) blocks = 4096;
+  planck_edge_kernel<<<(unsigned)blocks, 256, 0, (cudaStream_t)stream>>>(x_dev, n, yz_dev, xi_dev, is_y_dev);
+  CU(cudaGetLastError());
+  return MGRHD_OK;
+}
+
 int mgrhd_measure_dfma_peak(long long iters, double* fma_per_second) {
   if (!fma_per_second || iters < 8) return MGRHD_ERR_ARG;
   int dev = 0, sms = 0;
@@ -352,9 +477,11 @@ void mgrhd_free(mgrhd_ctx* ctx) {
   if (!ctx) return;
   for (int k = 0; k < kSlabs; ++k) {
     if (ctx->slab[k]) cudaFree(ctx->slab[k]);
+    if (ctx->slab_scratch[k]) cudaFree(ctx->slab_scratch[k]);
     if (ctx->slab_stream[k]) cudaStreamDestroy(ctx->slab_stream[k]);
   }
   if (ctx->d_stats) cudaFree(ctx->d_stats);
+  if (ctx->scratch) cudaFree(ctx->scratch);
   delete ctx;
 }
 

@@ -11,8 +11,6 @@
 namespace mgrhd {
 
 constexpr int kMaxG = MGRHD_MAX_GROUPS;
-constexpr int kSmallTerms = 16;   // even Maclaurin terms kept in the small-x edge functions
-constexpr int kSeriesMax = 40;    // longest exponential series (x >= kXSplit)
 
 // Device counters, one block of long long in global memory (see mgrhd_stats).
 enum StatSlot {
@@ -34,9 +32,9 @@ enum StatSlot {
 // (FMA = 2; add, mul, div, sqrt = 1; exp = kFlopExp; comparisons, fabs, selects = 0).
 // Derived line by line in DESIGN.md "Algorithmic flops"; used only by the counting kernels.
 constexpr int kFlopExp = 30;          // range reduction + degree-11 polynomial + scaling
-constexpr int kFlopEdgeSmall = 75;    // x < kXSplit: two 16-term Horner chains + assembly
-constexpr int kFlopEdgeLargeBase = 42;  // x >= kXSplit: exp, powers, Xi with one division
-constexpr int kFlopEdgeTerm = 11;     // one term of the e^{-nx} series
+constexpr int kFlopEdgeSmall = 59;    // x < kXS: two 12-term Horner chains in x^2 + assembly
+constexpr int kFlopEdgeMid = 95;      // kXS <= x < kXL: two degree-23 Horner chains
+constexpr int kFlopEdgeLarge = 94;    // x >= kXL: exp, 7 terms (3+1 FMA each), Xi with one reciprocal
 constexpr int kFlopEdgeZero = 32;     // e^{-x} underflowed
 constexpr int kFlopGroupEval = 62;    // a2-a5 for one group at one trial T
 constexpr int kFlopCellEval = 13;     // T, a_R T^4, beta, F_G, Eq. 49
@@ -62,6 +60,8 @@ struct Params {
   double k_hi[kMaxG];       // kappa_lo[g] * r_g^alpha_g         (chi_{g+}, Eq. 19 at nu_g+)
   double k_mean[kMaxG];     // kappa_lo[g] * (r^alpha-1)/(alpha ln r)   (Eq. 30 with alpha_Q=-1)
   double inv_k_mean[kMaxG]; // 1 / k_mean[g]
+  double k_num[kMaxG];      // k_mean[g] * (4 + alpha_g)/3 : numerator factor of Eq. 27 with chi_B = chi_E
+  double onepa[kMaxG];      // 1 + alpha_g (Eq. 21, 22)
   // ---- per call ------------------------------------------------------------------
   double dt, c, c_hat;
   long long ncells;   // cells in this launch
@@ -77,13 +77,23 @@ struct StatePtrs {
   const double* kappa_scale;  // may be null
 };
 
-// Small-x Maclaurin tables, filled by the host at first use (mgrhd_api.cu: fill_planck_tables)
-// and uploaded to __constant__ memory in the kernel translation unit.
+// Tables of the Planck edge functions (mgrhd_planck.cuh), filled by the host once per device
+// (mgrhd_api.cu: fill_planck_tables) and uploaded to __constant__ memory.
+constexpr int kSmallTerms = 12;   // even Maclaurin terms, x < kXS
+constexpr int kMidTerms = 24;     // monomial terms of the mid-range fits, kXS <= x < kXL
+constexpr int kLargeTerms = 7;    // terms of the e^{-nx} series, x >= kXL
+constexpr double kXS = 1.25;
+constexpr double kXL = 5.5;
 struct PlanckTables {
-  // t/(e^t-1) = 1 - t/2 + sum_{n>=1} b2n[n-1] t^(2n);  b_{2n} = B_{2n}/(2n)!
-  double xi_c[kSmallTerms];   // b_{2n}                     : Xi(x) = C x^3 (1 - x/2 + sum xi_c[n-1] x^(2n))
-  double y_c[kSmallTerms];    // b_{2n} / (2n+3)            : Y(x)  = C x^3 (1/3 - x/8 + sum y_c[n-1] x^(2n))
-  double inv_n[kSeriesMax + 1];  // 1/n, n = 1..kSeriesMax (index 0 unused)
+  // t/(e^t-1) = 1 - t/2 + sum_{n>=1} b_{2n} t^(2n),  b_{2n} = B_{2n}/(2n)!
+  double xi_c[kSmallTerms];   // b_{2n}          : Xi(x) = C x^3 (1 - x/2 + sum xi_c[n-1] x^(2n))
+  double y_c[kSmallTerms];    // b_{2n}/(2n+3)   : Y(x)  = C x^3 (1/3 - x/8 + sum y_c[n-1] x^(2n))
+  // mid range: Z(x) = sum mz[k] t^k, Xi(x) = sum mx[k] t^k, t = mid_s * x + mid_o in [-1, 1]
+  double mz[kMidTerms];
+  double mx[kMidTerms];
+  double mid_s, mid_o;
+  // large x: Z(x) = C sum_{n=1..kLargeTerms} e^{-nx} (x^3/n + 3x^2/n^2 + 6x/n^3 + 6/n^4)
+  double l3[kLargeTerms], l2[kLargeTerms], l1[kLargeTerms], l0[kLargeTerms];   // C/n, 3C/n^2, 6C/n^3, 6C/n^4
 };
 
 }  // namespace mgrhd

@@ -4,12 +4,17 @@
 //   Y(x)  = (15/pi^4) int_0^x t^3/(e^t-1) dt,   Z(x) = 1 - Y(x),
 //   Xi(x) = (15/pi^4) x^4/(e^x-1)               (4 pi nu B_nu / c = a_R T^4 Xi(x)).
 //
-// Each edge returns ONE of Y (x < kXSplit, Maclaurin series in x^2) or Z (x >= kXSplit,
-// sum_n e^{-nx}(x^3/n + 3x^2/n^2 + 6x/n^3 + 6/n^4)), so that a group difference never
-// cancels in the Wien tail:  both small: Y+ - Y-;  both large: Z- - Z+;  straddling:
-// 1 - Y- - Z+.
+// Each edge returns ONE of Y (x < kXS) or Z (x >= kXS), so that a group difference never
+// cancels in the Wien tail:  both Y: Y+ - Y-;  both Z: Z- - Z+;  straddling: 1 - Y- - Z+.
+// Three branches of BOUNDED cost (a warp evaluates one edge index at 32 temperatures, so the
+// lanes of a warp usually share a branch; when they do not, the warp pays the sum):
+//   x <  kXS        Maclaurin series in x^2, 12 even terms (truncation < 1e-19 relative);
+//   kXS <= x < kXL  degree-23 polynomial fits of Z and Xi (Chebyshev interpolants generated
+//                   in long double at init, abs. error < 1e-17 on functions of size 0.2-0.9);
+//   x >= kXL        u = e^{-x}; Z = C sum_{n<=7} u^n (x^3/n + 3x^2/n^2 + 6x/n^3 + 6/n^4)
+//                   (first dropped term < 3e-18 relative), Xi = C x^4 u/(1-u).
 //
-// Product code; independent of oracle/ (which sums in long double with a different split).
+// Product code; independent of oracle/ (which sums both series in long double, split at x=1).
 #pragma once
 #include "mgrhd_params.h"
 
@@ -17,8 +22,9 @@ namespace mgrhd {
 
 __constant__ PlanckTables c_planck;
 
-constexpr double kXSplit = 1.5;                       // series switch
 constexpr double kC15Pi4 = 0.15398973382026503;       // 15/pi^4
+
+__device__ __forceinline__ double fast_rcp(double x);  // mgrhd_kernels.cuh
 
 struct EdgeFn {
   double yz;   // Y(x) if small, else Z(x)
@@ -30,7 +36,7 @@ struct EdgeFn {
 // x in [0, +inf].  x == 0 -> (Y=0, Xi=0); x == +inf or e^-x == 0 -> (Z=0, Xi=0).
 __device__ __forceinline__ EdgeFn planck_edge(double x) {
   EdgeFn r;
-  if (x < kXSplit) {
+  if (x < kXS) {
     const double x2 = x * x;
     double sy = c_planck.y_c[kSmallTerms - 1];
     double sx = c_planck.xi_c[kSmallTerms - 1];
@@ -48,6 +54,20 @@ __device__ __forceinline__ EdgeFn planck_edge(double x) {
     return r;
   }
   r.small = false;
+  if (x < kXL) {
+    const double t = fma(x, c_planck.mid_s, c_planck.mid_o);
+    double sz = c_planck.mz[kMidTerms - 1];
+    double sx = c_planck.mx[kMidTerms - 1];
+#pragma unroll
+    for (int n = kMidTerms - 2; n >= 0; --n) {
+      sz = fma(sz, t, c_planck.mz[n]);
+      sx = fma(sx, t, c_planck.mx[n]);
+    }
+    r.yz = sz;
+    r.xi = sx;
+    r.flops = kFlopEdgeMid;
+    return r;
+  }
   const double u = exp(-x);
   if (!(u > 0.0)) {  // underflow or x = +inf
     r.yz = 0.0;
@@ -55,24 +75,16 @@ __device__ __forceinline__ EdgeFn planck_edge(double x) {
     r.flops = kFlopEdgeZero;
     return r;
   }
-  const double x2 = x * x, x3 = x2 * x;
-  const double c3 = x3, c2 = 3.0 * x2, c1 = 6.0 * x, c0 = 6.0;
-  double un = u;     // u^n
+  const double x2 = x * x;
   double sum = 0.0;
-  int nt = 0;
-  for (int n = 1; n <= kSeriesMax; ++n) {
-    const double q = c_planck.inv_n[n];
-    // x^3/n + 3x^2/n^2 + 6x/n^3 + 6/n^4  by Horner in 1/n
-    const double pn = q * fma(q, fma(q, fma(q, c0, c1), c2), c3);
-    const double term = un * pn;
-    sum += term;
-    ++nt;
-    if (term <= 1e-18 * sum) break;
-    un *= u;
+#pragma unroll
+  for (int n = kLargeTerms - 1; n >= 0; --n) {
+    const double pn = fma(fma(fma(c_planck.l3[n], x, c_planck.l2[n]), x, c_planck.l1[n]), x, c_planck.l0[n]);
+    sum = fma(sum, u, pn);
   }
-  r.yz = kC15Pi4 * sum;
-  r.xi = kC15Pi4 * (x2 * x2) * (u / (1.0 - u));
-  r.flops = kFlopEdgeLargeBase + kFlopEdgeTerm * nt;
+  r.yz = sum * u;
+  r.xi = kC15Pi4 * (x2 * x2) * (u * fast_rcp(1.0 - u));
+  r.flops = kFlopEdgeLarge;
   return r;
 }
 
