@@ -71,17 +71,26 @@ __device__ __forceinline__ void closure_vP(int closure, double E, double F0, dou
 }
 
 // Lane phases of the flattened iteration.
-enum Phase : int { PH_LOAD = 0, PH_EVAL = 1, PH_FLUX = 2, PH_STORE = 3, PH_DONE = 4 };
+enum Phase : int { PH_LOAD = 0, PH_EVAL = 1, PH_FLUX = 2, PH_DONE = 3 };
 
-// Shared-memory slots (per thread, per group).
+// Per-thread, per-group slots.  DA/DB/AG are reused for F_g^(new) between the two flux passes.
 enum Slot : int { SL_R = 0, SL_DA, SL_DB, SL_VF, SL_AG, SL_CHIF, SL_COUNT };
-
 
 // NQ: compile-time group capacity (runtime Nq <= NQ); THREADS: CTA size; NSMEM: how many of the
 // SL_COUNT per-group slots live in shared memory (the rest go to the global scratch).
 // Dynamic shared memory: NSMEM * NQ * THREADS doubles.
-// scratch: (3 + SL_COUNT - NSMEM) * NQ * (gridDim.x*THREADS) doubles of global memory (the lagged
-// fluxes F_g,k and the overflow slots), private to this launch.
+// scratch: (3 + SL_COUNT - NSMEM) * NQ * (gridDim.x*THREADS) doubles of global memory, private to
+// this launch: F_g^(t) of the cell in flight (the state's Frad holds the lagged F_g,k in place)
+// and the overflow slots.
+//
+// One trip of the main loop, per warp (all loops over groups are entered warp-wide):
+//   LOAD  lanes without a cell take the next cells of the warp's chunk (scalars only);
+//   A     every lane with a cell evaluates all groups at its trial T (a1-a5); the Newton update
+//         of R_g decided in the previous trip is applied on the fly, the first evaluation of a
+//         cell also forms v.F_g and sum E_g, and a lane that has just finished a cell stores
+//         that cell's E_g here, so neither costs a loop of its own;
+//   B, C  lanes whose Newton iteration converged do the flux/momentum update and the outer test
+//         (a6-a9); F_g is updated in place in the state, so a finished cell needs no flux store.
 template <int NQ, int THREADS, int NSMEM, bool COUNT>
 __global__ void __launch_bounds__(THREADS, 1)
 source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ StatePtrs S,
@@ -97,23 +106,23 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
   const long long n = P.ncells, stride = P.stride;
   const double dt = P.dt, c = P.c, chat = P.c_hat;
   const double c_over_chat = c / chat, inv_c = 1.0 / c, cdt = chat * dt, icc = 1.0 / (c * chat);
+  const double rel2 = P.outer_rel_tol * P.outer_rel_tol;
 
-  // shared-memory slot s, group g of this thread
+  const long long tthreads = (long long)gridDim.x * THREADS;
+  const long long gtid = (long long)blockIdx.x * THREADS + tid;
+  // slot s, group g of this thread: shared memory, or global scratch for the overflow slots
   auto sm = [&](int s, int g) -> double& {
     if (s < NSMEM) return smem[(s * NQ + g) * THREADS + tid];
-    return scratch[(long long)((3 + s - NSMEM) * NQ + g) * ((long long)gridDim.x * THREADS) +
-                   ((long long)blockIdx.x * THREADS + tid)];
+    return scratch[(long long)((3 + s - NSMEM) * NQ + g) * tthreads + gtid];
   };
-  // lagged flux component i, group g of this thread (global scratch, coalesced across the warp)
-  const long long tthreads = (long long)gridDim.x * THREADS;
-  double* const fk_base = scratch + ((long long)blockIdx.x * THREADS + tid);
-  auto fk = [&](int i, int g) -> double& { return fk_base[(long long)(i * NQ + g) * tthreads]; };
+  // F_g^(t), component i, of the cell in flight (global scratch, coalesced across the warp)
+  auto ft = [&](int i, int g) -> double& { return scratch[(long long)(i * NQ + g) * tthreads + gtid]; };
 
   // this warp's contiguous chunk of cells [next, end)
-  const long long nwarps = tthreads >> 5, wid = ((long long)blockIdx.x * THREADS + tid) >> 5;
+  const long long nwarps = tthreads >> 5, wid = gtid >> 5;
   const long long per = (n + nwarps - 1) / nwarps;
   long long next = wid * per;
-  long long end = next + per < n ? next + per : n;
+  const long long end = next + per < n ? next + per : n;
   if (next > n) next = n;
 
   unsigned int cnt_newton_unconv = 0, cnt_outer_unconv = 0, cnt_Tnonpos = 0, cnt_guard = 0,
@@ -122,14 +131,30 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
 
   // ---- per-lane cell state -----------------------------------------------------------------
   int phase = PH_LOAD;
-  long long cell = -1;
-  double rho = 1.0, chis = 1.0, inv_chis = 1.0, Cv = 1.0, inv_Cv = 1.0, Egas_t = 0.0, Etot = 1.0;
-  double momt0 = 0, momt1 = 0, momt2 = 0, momk0 = 0, momk1 = 0, momk2 = 0, momn0 = 0, momn1 = 0, momn2 = 0;
-  double Egs = 0.0, Egas_new = 0.0, Ekin = 0.0;
+  long long cell = 0, fin_cell = -1;   // fin_cell: finished cell whose E_g store is still due
+  double rho = 1.0, inv_rho = 1.0, chis = 1.0, inv_chis = 1.0, inv_Cv = 1.0, Egas_t = 0.0, Etot = 1.0;
+  double momt0 = 0, momt1 = 0, momt2 = 0, momk0 = 0, momk1 = 0, momk2 = 0;
+  double Egs = 0.0, Ekin = 0.0, lam = 0.0, ldx = 0.0;
+  bool first = false, pend = false;
   int it = 0, k = 0, evals = 0, trips = 0;
 
+  // a cell is finished: counters, scalar stores; its E_g store is done in the next loop A
+  auto finish = [&](double mn0, double mn1, double mn2, double Egas_new) {
+    if (trips > 0) {
+      S.mom[0][cell] = mn0; S.mom[1][cell] = mn1; S.mom[2][cell] = mn2;
+      S.Egas[cell] = Egas_new;   // total gas energy; E_int = Egas - |mom|^2/(2 rho)
+      fin_cell = cell;
+    }
+    cnt_evals += evals;
+    cnt_trips += trips;
+    cnt_cells++;
+    atomicAdd(&s_hist[evals < MGRHD_HIST ? evals : MGRHD_HIST - 1], 1u);
+    atomicAdd(&s_hist[MGRHD_HIST + (trips < MGRHD_HIST ? trips : MGRHD_HIST - 1)], 1u);
+    phase = PH_LOAD;
+  };
+
   while (true) {
-    // ===== LOAD: lanes that need a cell take the next ones of the warp's chunk (a0) ===========
+    // ===== LOAD (a0): scalars of the next cell of the warp's chunk ================================
     const unsigned need = __ballot_sync(FULL, phase == PH_LOAD);
     if (need) {
       if (phase == PH_LOAD) {
@@ -138,43 +163,37 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
           cell = cnew;
           rho = S.rho[cell];
           const double ks = S.kappa_scale ? S.kappa_scale[cell] : 1.0;
-          chis = rho * ks;                      // chi_{g-} = chis * k_lo[g]
-          inv_chis = 1.0 / chis;
-          Cv = rho * P.cv_over_rho;
-          inv_Cv = 1.0 / Cv;
           momt0 = S.mom[0][cell]; momt1 = S.mom[1][cell]; momt2 = S.mom[2][cell];
           Egas_t = S.Egas[cell];
-          const double inv_rho = 1.0 / rho;
-          const double v0 = momt0 * inv_rho, v1 = momt1 * inv_rho, v2 = momt2 * inv_rho;
-          double sumEt = 0.0;
-          for (int g = 0; g < Nq; ++g) {
-            const long long o = (long long)g * stride + cell;
-            const double F0 = S.Frad[0][o], F1 = S.Frad[1][o], F2 = S.Frad[2][o];
-            sumEt += S.Erad[o];
-            fk(0, g) = F0; fk(1, g) = F1; fk(2, g) = F2;
-            sm(SL_R, g) = 0.0;
-            sm(SL_VF, g) = fma(v0, F0, fma(v1, F1, v2 * F2));   // lagged v.F_g of the first trip
-          }
-          Etot = Egas_t + (chat / c) * sumEt;   // Eq. 50 as printed, S_g = 0
-          momk0 = momn0 = momt0; momk1 = momn1 = momt1; momk2 = momn2 = momt2;
-          Egs = Egas_new = Egas_t;
-          Ekin = (momk0 * momk0 + momk1 * momk1 + momk2 * momk2) / (2.0 * rho);
+          chis = rho * ks;                      // chi_{g-} = chis * k_lo[g]
+          inv_chis = 1.0 / chis;
+          inv_rho = 1.0 / rho;
+          inv_Cv = 1.0 / (rho * P.cv_over_rho);
+          momk0 = momt0; momk1 = momt1; momk2 = momt2;
+          Egs = Egas_t;
+          Ekin = (momk0 * momk0 + momk1 * momk1 + momk2 * momk2) * (0.5 * inv_rho);
           it = 0; k = 0; evals = 0; trips = 0;
+          first = true; pend = false;
           if (COUNT) flops += kFlopCell + kFlopCellGroup * Nq;
-          if ((Egs - Ekin) * inv_Cv > 0.0) phase = PH_EVAL;
-          else { cnt_Tnonpos++; phase = PH_STORE; }     // invalid state: leave the cell as it is
+          if ((Egs - Ekin) * inv_Cv > 0.0) {
+            phase = PH_EVAL;
+          } else {                              // invalid state: count it, leave the cell as it is
+            cnt_Tnonpos++;
+            finish(0.0, 0.0, 0.0, 0.0);
+          }
         } else {
           phase = PH_DONE;
-          cell = -1;
         }
       }
       next += __popc(need);
     }
     if (__all_sync(FULL, phase == PH_DONE)) break;
 
-    // ===== EVAL: all groups at the trial temperature (a1-a5), then Eq. 49 ========================
-    if (phase == PH_EVAL) {
-      const double T = (Egs - Ekin) * inv_Cv;
+    // ===== A: all groups at the trial temperature (a1-a5), then Eq. 49 ============================
+    if (__any_sync(FULL, phase == PH_EVAL)) {
+      const bool ev = phase == PH_EVAL;
+      const bool fin = fin_cell >= 0;
+      const double T = ev ? (Egs - Ekin) * inv_Cv : 1.0;
       const double invT = 1.0 / T;
       const double T2 = T * T;
       const double aT4 = P.a_rad * T2 * T2;
@@ -182,175 +201,224 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
       const double itau_c = inv_chis / cdt;          // 1/(c_hat dt chi_E,g) = itau_c * inv_k_mean[g]
       const double dBscale = invT * inv_Cv;          // J_g0 = (4 Bt - Db) / (T C_v), Eq. 46
       const double guard_thr = 1e-280 * aT4;
-      double sumR = 0.0, sumAbsFR = 0.0, SFRq = 0.0, SJq = 0.0;
-      EdgeFn lo = planck_edge(P.nu[0] * beta);
-      if (COUNT) flops += kFlopCellEval + lo.flops + (unsigned)(kFlopGroupEval * Nq);
-      double Et_next = S.Erad[cell];
-      for (int g = 0; g < Nq; ++g) {
-        // a1: edge functions at the upper edge of group g
-        const EdgeFn hi = planck_edge(P.nu[g + 1] * beta);
-        if (COUNT) flops += hi.flops;
-        const double Et = Et_next;
-        if (g + 1 < Nq) Et_next = S.Erad[(long long)(g + 1) * stride + cell];
-        // a2: group Planck integral and Doppler boundary terms (Eq. 11, 18, 22)
-        const double Bt = aT4 * planck_dY(lo, hi);
-        const double Db = aT4 * (hi.xi - lo.xi);
-        const double D = aT4 * chis * fma(P.k_hi[g], hi.xi, -P.k_lo[g] * lo.xi);
-        const double chiE = chis * P.k_mean[g];                  // = chi_B (alpha_Q = -1 for both)
-        const double fourBmDb = fma(4.0, Bt, -Db);               // = 3 * denominator of Eq. 27 = T dBt/dT
-        // a3: flux-mean opacity, Eq. 27, with the Wien-limit guard (S8)
-        const double den = fourBmDb * (1.0 / 3.0);
-        const double num = fma(chis * Bt, P.k_num[g], -D * (1.0 / 3.0));   // (chi_B+chi_E/3+alpha chi_E/3) Bt - D/3
-        double chiF;
-        if (!(den >= guard_thr) || isinf(den)) {
-          chiF = chis * P.k_lo[g];
-          if (evals == 0) cnt_guard++;
-        } else if (den > 1e-290 && den < 1e290) {
-          chiF = num * fast_rcp(den);
-        } else {
-          chiF = num / den;
-        }
-        if (!(fma(cdt, chiF, 1.0) > 0.0)) {
-          if (evals == 0) cnt_den++;
-          chiF = chiE;
-        }
-        // a4: residuals (Eq. 41; Eq. 42 solved for E_g)
-        const double R = sm(SL_R, g);
-        const double inv_chiE = inv_chis * P.inv_k_mean[g];
-        const double itau = itau_c * P.inv_k_mean[g];
-        const double W = P.onepa[g] * chiF * sm(SL_VF, g) * inv_c;
-        const double Eg = fma(W * inv_chiE, inv_c, Bt) - R * itau;
-        const double FR = Eg - Et - R;
-        sumR += R;
-        sumAbsFR += fabs(FR);
-        // a5: Jacobian pieces (Eq. 44-47) folded into the arrowhead elimination (Eq. 48):
-        //     1/J_gg = -q, q = 1/(1 + itau)
-        const double q = fast_rcp(1.0 + itau);
-        const double Jg0 = fourBmDb * dBscale;
-        const double da = FR * q, db = Jg0 * q;
-        SFRq += da;
-        SJq += db;
-        sm(SL_DA, g) = da;
-        sm(SL_DB, g) = db;
-        sm(SL_AG, g) = fma(chiE, Bt, -D * (1.0 / 3.0));          // chi_B Bt - D/3 (Eq. 51 source)
-        sm(SL_CHIF, g) = chiF;
-        lo = hi;
-      }
-      const double FG = Egs - Egas_t + c_over_chat * sumR;
-      evals++;
-      const double inv_Etot = 1.0 / Etot;
-      if (fabs(FG) * inv_Etot < P.newton_tol && c_over_chat * sumAbsFR * inv_Etot < P.newton_tol) {
-        phase = PH_FLUX;                                          // Eq. 49 met
-      } else if (it >= P.newton_maxit) {
-        cnt_newton_unconv++;
-        phase = PH_FLUX;
-      } else {
-        // Newton step: eliminate the gas row
-        //   dx0 = (-F_G + sum J0g F_R,g/Jgg) / (1 - sum J0g Jg0/Jgg),  dR_g = (F_R,g + Jg0 dx0) q
-        const double dx0 = (-FG - c_over_chat * SFRq) / fma(c_over_chat, SJq, 1.0);
-        double lam = 1.0;
-        for (int h = 0; h < 10 && !((Egs + lam * dx0 - Ekin) * inv_Cv > 0.0); ++h) {
-          lam *= 0.5;
-          cnt_Tnonpos++;
-        }
-        Egs += lam * dx0;
-        const double ldx = lam * dx0;
-        for (int g = 0; g < Nq; ++g) sm(SL_R, g) = fma(lam, sm(SL_DA, g), fma(ldx, sm(SL_DB, g), sm(SL_R, g)));
-        it++;
-        if (COUNT) flops += kFlopStepCell + kFlopStepGroup * Nq;
-      }
-    }
-
-    // ===== FLUX: energy commit (a6), closure + Eq. 51 (a7), Eq. 52 (a8), outer test (a9) =========
-    if (phase == PH_FLUX) {
-      const double inv_rho = 1.0 / rho;
       const double v0 = momk0 * inv_rho, v1 = momk1 * inv_rho, v2 = momk2 * inv_rho;
-      double sumR = 0.0, dF0 = 0.0, dF1 = 0.0, dF2 = 0.0;
-      bool rel_ok = true;
+      double sumR = 0.0, sumAbsFR = 0.0, SFRq = 0.0, SJq = 0.0, sumEt = 0.0;
+      EdgeFn lo;
+      if (ev) {
+        lo = planck_edge(P.nu[0] * beta);
+        if (COUNT) flops += kFlopCellEval + lo.flops + (unsigned)(kFlopGroupEval * Nq);
+      }
+      // software prefetch of the next group's global operands
+      double nEt = 0.0, nF0 = 0.0, nF1 = 0.0, nF2 = 0.0, nEo = 0.0;
+      if (ev) nEt = S.Erad[cell];
+      if (ev && first) { nF0 = S.Frad[0][cell]; nF1 = S.Frad[1][cell]; nF2 = S.Frad[2][cell]; }
+      if (fin) nEo = S.Erad[fin_cell];
       for (int g = 0; g < Nq; ++g) {
-        const long long o = (long long)g * stride + cell;
-        const double Ft0 = S.Frad[0][o], Ft1 = S.Frad[1][o], Ft2 = S.Frad[2][o];
-        const double Fk0 = fk(0, g), Fk1 = fk(1, g), Fk2 = fk(2, g);
-        const double R = sm(SL_R, g);
-        sumR += R;
-        const double Enew = S.Erad[o] + R;                        // E_g^(t+1) = E_g^(t) + R_g
-        double p0, p1, p2;
-        closure_vP(P.closure, Enew, Fk0, Fk1, Fk2, v0, v1, v2, c, p0, p1, p2);
-        const double w = P.onepa[g] * (chis * P.k_mean[g]);       // (1 + alpha) chi_E
-        const double chiF = sm(SL_CHIF, g), A = sm(SL_AG, g);
-        const double dn = fma(cdt, chiF, 1.0);                    // 1 + c_hat chi_F dt > 0 (guarded in EVAL)
-        const double inv_dn = (dn > 1e-290 && dn < 1e290) ? fast_rcp(dn) : 1.0 / dn;
-        const double Fn0 = fma(cdt, fma(v0, A, w * p0), Ft0) * inv_dn;
-        const double Fn1 = fma(cdt, fma(v1, A, w * p1), Ft1) * inv_dn;
-        const double Fn2 = fma(cdt, fma(v2, A, w * p2), Ft2) * inv_dn;
-        dF0 += Fn0 - Ft0; dF1 += Fn1 - Ft1; dF2 += Fn2 - Ft2;
-        if (P.outer_stop == 1) {
-          const double e0 = Fn0 - Fk0, e1 = Fn1 - Fk1, e2 = Fn2 - Fk2;
-          const double d2 = fma(e0, e0, fma(e1, e1, e2 * e2));
-          const double f2 = fma(Fn0, Fn0, fma(Fn1, Fn1, Fn2 * Fn2));
-          // |dF| <= rel |F|  (compared squared unless the squares leave the normal range)
-          bool ok;
-          if (f2 > 1e-280 && f2 < 1e280) ok = d2 <= P.outer_rel_tol * P.outer_rel_tol * f2;
-          else ok = norm3(e0, e1, e2) <= P.outer_rel_tol * norm3(Fn0, Fn1, Fn2);
-          if (!ok) rel_ok = false;
+        const double Et = nEt, F0 = nF0, F1 = nF1, F2 = nF2, Eo = nEo;
+        if (g + 1 < Nq) {
+          const long long o1 = (long long)(g + 1) * stride;
+          if (ev) nEt = S.Erad[o1 + cell];
+          if (ev && first) { nF0 = S.Frad[0][o1 + cell]; nF1 = S.Frad[1][o1 + cell]; nF2 = S.Frad[2][o1 + cell]; }
+          if (fin) nEo = S.Erad[o1 + fin_cell];
         }
-        fk(0, g) = Fn0; fk(1, g) = Fn1; fk(2, g) = Fn2;
+        // a10 of the cell this lane finished in the previous trip: E_g^(t+1) = E_g^(t) + R_g
+        if (fin) S.Erad[(long long)g * stride + fin_cell] = Eo + sm(SL_R, g);
+        if (ev) {
+          // a1: edge functions at the upper edge of group g
+          const EdgeFn hi = planck_edge(P.nu[g + 1] * beta);
+          if (COUNT) flops += hi.flops;
+          // R_g and the lagged v.F_g
+          double R, vF;
+          if (first) {
+            R = 0.0;
+            vF = fma(v0, F0, fma(v1, F1, v2 * F2));
+            sumEt += Et;
+            sm(SL_R, g) = 0.0;
+            sm(SL_VF, g) = vF;
+          } else {
+            R = sm(SL_R, g);
+            if (pend) {     // Newton update decided at the end of the previous evaluation (Eq. 48)
+              R = fma(lam, sm(SL_DA, g), fma(ldx, sm(SL_DB, g), R));
+              sm(SL_R, g) = R;
+            }
+            vF = sm(SL_VF, g);
+          }
+          // a2: group Planck integral and Doppler boundary terms (Eq. 11, 18, 22)
+          const double Bt = aT4 * planck_dY(lo, hi);
+          const double Db = aT4 * (hi.xi - lo.xi);
+          const double D = aT4 * chis * fma(P.k_hi[g], hi.xi, -P.k_lo[g] * lo.xi);
+          const double chiE = chis * P.k_mean[g];                  // = chi_B (alpha_Q = -1 for both)
+          const double fourBmDb = fma(4.0, Bt, -Db);               // 3 x denominator of Eq. 27 = T dBt/dT
+          // a3: flux-mean opacity, Eq. 27, with the Wien-limit guard (S8)
+          const double den = fourBmDb * (1.0 / 3.0);
+          const double Dthird = D * (1.0 / 3.0);
+          const double num = fma(chis * Bt, P.k_num[g], -Dthird);  // (chi_B + chi_E/3 + alpha chi_E/3) Bt - D/3
+          double chiF;
+          if (!(den >= guard_thr) || isinf(den)) {
+            chiF = chis * P.k_lo[g];
+            if (evals == 0) cnt_guard++;
+          } else if (den > 1e-290 && den < 1e290) {
+            chiF = num * fast_rcp(den);
+          } else {
+            chiF = num / den;
+          }
+          if (!(fma(cdt, chiF, 1.0) > 0.0)) {
+            if (evals == 0) cnt_den++;
+            chiF = chiE;
+          }
+          // a4: residuals (Eq. 41; Eq. 42 solved for E_g)
+          const double inv_chiE = inv_chis * P.inv_k_mean[g];
+          const double itau = itau_c * P.inv_k_mean[g];
+          const double W = P.onepa[g] * chiF * vF * inv_c;
+          const double Eg = fma(W * inv_chiE, inv_c, Bt) - R * itau;
+          const double FR = Eg - Et - R;
+          sumR += R;
+          sumAbsFR += fabs(FR);
+          // a5: Jacobian (Eq. 44-47) folded into the arrowhead elimination (Eq. 48): 1/J_gg = -q
+          const double q = fast_rcp(1.0 + itau);
+          const double da = FR * q, db = fourBmDb * dBscale * q;
+          SFRq += da;
+          SJq += db;
+          sm(SL_DA, g) = da;
+          sm(SL_DB, g) = db;
+          sm(SL_AG, g) = fma(chiE, Bt, -Dthird);                   // chi_B Bt - D/3 (Eq. 51 source)
+          sm(SL_CHIF, g) = chiF;
+          lo = hi;
+        }
       }
-      Egas_new = Egas_t - c_over_chat * sumR;
-      momn0 = momt0 - dF0 * icc; momn1 = momt1 - dF1 * icc; momn2 = momt2 - dF2 * icc;   // Eq. 52
-      trips++;
-      if (COUNT) flops += kFlopOuterCell + kFlopOuterGroup * Nq;
-
-      const double vn0 = momn0 * inv_rho, vn1 = momn1 * inv_rho, vn2 = momn2 * inv_rho;
-      double dW = 0.0, sumAbsR = 0.0;
-      for (int g = 0; g < Nq; ++g) {
-        const double vFn = fma(vn0, fk(0, g), fma(vn1, fk(1, g), vn2 * fk(2, g)));
-        const double wf = P.onepa[g] * sm(SL_CHIF, g) * inv_c;
-        dW += fabs(wf * (vFn - sm(SL_VF, g)));
-        sumAbsR += fabs(sm(SL_R, g));
-        sm(SL_VF, g) = vFn;                                       // lagged v.F_g of the next trip
-      }
-      if (P.outer_stop == 1) {
-        const double d = norm3(momn0 - momk0, momn1 - momk1, momn2 - momk2);
-        if (!(d <= P.outer_rel_tol * norm3(momn0, momn1, momn2))) rel_ok = false;
-      }
-      const double delta = dW * (chat / c) * dt;
-      if (delta <= P.outer_tol * fmax(sumAbsR, Etot) && rel_ok) {
-        phase = PH_STORE;
-      } else if (k == P.outer_maxit - 1) {
-        cnt_outer_unconv++;
-        phase = PH_STORE;
-      } else {
-        momk0 = momn0; momk1 = momn1; momk2 = momn2;
-        Ekin = (momk0 * momk0 + momk1 * momk1 + momk2 * momk2) / (2.0 * rho);
-        k++;
-        it = 0;
-        if ((Egs - Ekin) * inv_Cv > 0.0) phase = PH_EVAL;
-        else { cnt_Tnonpos++; phase = PH_STORE; }
+      fin_cell = fin ? -1 : fin_cell;
+      if (ev) {
+        if (first) Etot = Egas_t + (chat / c) * sumEt;             // Eq. 50 as printed, S_g = 0
+        first = false;
+        pend = false;
+        const double FG = Egs - Egas_t + c_over_chat * sumR;
+        evals++;
+        const double inv_Etot = 1.0 / Etot;
+        if (fabs(FG) * inv_Etot < P.newton_tol && c_over_chat * sumAbsFR * inv_Etot < P.newton_tol) {
+          phase = PH_FLUX;                                          // Eq. 49 met
+        } else if (it >= P.newton_maxit) {
+          cnt_newton_unconv++;
+          phase = PH_FLUX;
+        } else {
+          // Newton step: eliminate the gas row
+          //   dx0 = (-F_G + sum J0g F_R,g/Jgg) / (1 - sum J0g Jg0/Jgg),  dR_g = (F_R,g + Jg0 dx0) q
+          const double dx0 = (-FG - c_over_chat * SFRq) / fma(c_over_chat, SJq, 1.0);
+          lam = 1.0;
+          for (int h = 0; h < 10 && !((Egs + lam * dx0 - Ekin) * inv_Cv > 0.0); ++h) {
+            lam *= 0.5;
+            cnt_Tnonpos++;
+          }
+          Egs += lam * dx0;
+          ldx = lam * dx0;
+          pend = true;          // R_g += lam da_g + ldx db_g, applied by the next evaluation
+          it++;
+          if (COUNT) flops += kFlopStepCell + kFlopStepGroup * Nq;
+        }
       }
     }
 
-    // ===== STORE (a10) ============================================================================
-    if (phase == PH_STORE) {
-      if (trips > 0) {
-        S.mom[0][cell] = momn0; S.mom[1][cell] = momn1; S.mom[2][cell] = momn2;
-        S.Egas[cell] = Egas_new;   // total gas energy; E_int = Egas - |mom|^2/(2 rho)
-        for (int g = 0; g < Nq; ++g) {
+    // ===== B, C: energy commit (a6), closure + Eq. 51 (a7), Eq. 52 (a8), outer test (a9) ==========
+    if (__any_sync(FULL, phase == PH_FLUX)) {
+      const bool fx = phase == PH_FLUX;
+      const bool t0 = trips == 0;       // first trip: F_g^(t) is still in the state, save it to the scratch
+      const double v0 = momk0 * inv_rho, v1 = momk1 * inv_rho, v2 = momk2 * inv_rho;
+      double sumR = 0.0, sumAbsR = 0.0, dF0 = 0.0, dF1 = 0.0, dF2 = 0.0;
+      bool rel_ok = true;
+      double nEt = 0.0, nFt0 = 0.0, nFt1 = 0.0, nFt2 = 0.0, nFk0 = 0.0, nFk1 = 0.0, nFk2 = 0.0;
+      if (fx) {
+        nEt = S.Erad[cell];
+        nFk0 = S.Frad[0][cell]; nFk1 = S.Frad[1][cell]; nFk2 = S.Frad[2][cell];
+        if (!t0) { nFt0 = ft(0, 0); nFt1 = ft(1, 0); nFt2 = ft(2, 0); }
+      }
+      for (int g = 0; g < Nq; ++g) {
+        const double Et = nEt, Fk0 = nFk0, Fk1 = nFk1, Fk2 = nFk2;
+        const double Ft0 = t0 ? nFk0 : nFt0, Ft1 = t0 ? nFk1 : nFt1, Ft2 = t0 ? nFk2 : nFt2;
+        if (fx && g + 1 < Nq) {
+          const long long o1 = (long long)(g + 1) * stride + cell;
+          nEt = S.Erad[o1];
+          nFk0 = S.Frad[0][o1]; nFk1 = S.Frad[1][o1]; nFk2 = S.Frad[2][o1];
+          if (!t0) { nFt0 = ft(0, g + 1); nFt1 = ft(1, g + 1); nFt2 = ft(2, g + 1); }
+        }
+        if (fx) {
           const long long o = (long long)g * stride + cell;
-          S.Erad[o] = S.Erad[o] + sm(SL_R, g);
-          S.Frad[0][o] = fk(0, g);
-          S.Frad[1][o] = fk(1, g);
-          S.Frad[2][o] = fk(2, g);
+          const double R = sm(SL_R, g);
+          sumR += R;
+          sumAbsR += fabs(R);
+          const double Enew = Et + R;                               // E_g^(t+1) = E_g^(t) + R_g
+          double p0, p1, p2;
+          closure_vP(P.closure, Enew, Fk0, Fk1, Fk2, v0, v1, v2, c, p0, p1, p2);
+          const double w = P.onepa[g] * (chis * P.k_mean[g]);       // (1 + alpha) chi_E
+          const double chiF = sm(SL_CHIF, g), A = sm(SL_AG, g);
+          const double dn = fma(cdt, chiF, 1.0);                    // 1 + c_hat chi_F dt > 0 (guarded in A)
+          const double inv_dn = (dn > 1e-290 && dn < 1e290) ? fast_rcp(dn) : 1.0 / dn;
+          const double Fn0 = fma(cdt, fma(v0, A, w * p0), Ft0) * inv_dn;
+          const double Fn1 = fma(cdt, fma(v1, A, w * p1), Ft1) * inv_dn;
+          const double Fn2 = fma(cdt, fma(v2, A, w * p2), Ft2) * inv_dn;
+          dF0 += Fn0 - Ft0; dF1 += Fn1 - Ft1; dF2 += Fn2 - Ft2;
+          if (P.outer_stop == 1) {
+            const double e0 = Fn0 - Fk0, e1 = Fn1 - Fk1, e2 = Fn2 - Fk2;
+            const double d2 = fma(e0, e0, fma(e1, e1, e2 * e2));
+            const double f2 = fma(Fn0, Fn0, fma(Fn1, Fn1, Fn2 * Fn2));
+            // |dF| <= rel |F|, compared squared unless the squares leave the normal range
+            bool ok;
+            if (f2 > 1e-280 && f2 < 1e280) ok = d2 <= rel2 * f2;
+            else ok = norm3(e0, e1, e2) <= P.outer_rel_tol * norm3(Fn0, Fn1, Fn2);
+            if (!ok) rel_ok = false;
+          }
+          if (t0) { ft(0, g) = Ft0; ft(1, g) = Ft1; ft(2, g) = Ft2; }
+          S.Frad[0][o] = Fn0; S.Frad[1][o] = Fn1; S.Frad[2][o] = Fn2;   // lagged flux of the next trip, in place
+          sm(SL_DA, g) = Fn0; sm(SL_DB, g) = Fn1; sm(SL_AG, g) = Fn2;   // kept on chip for loop C
         }
       }
-      cnt_evals += evals;
-      cnt_trips += trips;
-      cnt_cells++;
-      atomicAdd(&s_hist[evals < MGRHD_HIST ? evals : MGRHD_HIST - 1], 1u);
-      atomicAdd(&s_hist[MGRHD_HIST + (trips < MGRHD_HIST ? trips : MGRHD_HIST - 1)], 1u);
-      phase = PH_LOAD;
+      double momn0 = 0.0, momn1 = 0.0, momn2 = 0.0, dW = 0.0;
+      if (fx) {
+        momn0 = momt0 - dF0 * icc; momn1 = momt1 - dF1 * icc; momn2 = momt2 - dF2 * icc;   // Eq. 52
+        trips++;
+        if (COUNT) flops += kFlopOuterCell + kFlopOuterGroup * Nq;
+      }
+      const double vn0 = momn0 * inv_rho, vn1 = momn1 * inv_rho, vn2 = momn2 * inv_rho;
+      for (int g = 0; g < Nq; ++g) {
+        if (fx) {
+          const double vFn = fma(vn0, sm(SL_DA, g), fma(vn1, sm(SL_DB, g), vn2 * sm(SL_AG, g)));
+          const double wf = P.onepa[g] * sm(SL_CHIF, g) * inv_c;
+          dW += fabs(wf * (vFn - sm(SL_VF, g)));
+          sm(SL_VF, g) = vFn;                                       // lagged v.F_g of the next trip
+        }
+      }
+      if (fx) {
+        const double Egas_new = Egas_t - c_over_chat * sumR;
+        if (P.outer_stop == 1) {
+          const double d = norm3(momn0 - momk0, momn1 - momk1, momn2 - momk2);
+          if (!(d <= P.outer_rel_tol * norm3(momn0, momn1, momn2))) rel_ok = false;
+        }
+        const double delta = dW * (chat / c) * dt;
+        if (delta <= P.outer_tol * fmax(sumAbsR, Etot) && rel_ok) {
+          finish(momn0, momn1, momn2, Egas_new);
+        } else if (k == P.outer_maxit - 1) {
+          cnt_outer_unconv++;
+          finish(momn0, momn1, momn2, Egas_new);
+        } else {
+          momk0 = momn0; momk1 = momn1; momk2 = momn2;
+          Ekin = (momk0 * momk0 + momk1 * momk1 + momk2 * momk2) * (0.5 * inv_rho);
+          k++;
+          it = 0;
+          if ((Egs - Ekin) * inv_Cv > 0.0) {
+            phase = PH_EVAL;
+          } else {
+            cnt_Tnonpos++;
+            finish(momn0, momn1, momn2, Egas_new);
+          }
+        }
+      }
     }
   }
+
+  // E_g store of the last cell of each lane (no further loop A ran for it)
+  if (fin_cell >= 0)
+    for (int g = 0; g < Nq; ++g) {
+      const long long o = (long long)g * stride + fin_cell;
+      S.Erad[o] = S.Erad[o] + sm(SL_R, g);
+    }
 
   // ---- diagnostics: warp-reduce the scalar counters, one atomic per warp ------------------
   unsigned int vals[8] = {cnt_cells, cnt_newton_unconv, cnt_outer_unconv, cnt_Tnonpos,
