@@ -139,7 +139,7 @@ struct mgrhd_ctx {
   cudaStream_t last_stream;
   long long launches;
   int count_flops;
-  int variant, cfg_nsmem;
+  int variant, cfg_l;
   int cfg_nq, cfg_threads, cfg_bps;   // kernel instantiation, CTA size, resident CTAs per SM
   double* scratch;                    // lagged-flux scratch of the device path
   double* slab_scratch[kSlabs];       // ... and of each host-path slab stream
@@ -149,42 +149,45 @@ struct mgrhd_ctx {
   cudaStream_t slab_stream[kSlabs];
 };
 
-// One instantiation per group capacity: CTA size chosen so the [slot][group][thread] state fits
-// in shared memory (SL_COUNT * NQ * THREADS * 8 bytes <= 192 KB).
-template <int NQ, int THREADS, int NSMEM>
+// One instantiation per (lanes per cell L, steps per lane NQL, CTA size): chosen so that the
+// [slot][step][thread] state fits in shared memory (SL_COUNT * NQL * THREADS * 8 bytes <= 227 KB)
+// with as many threads per SM as the register file allows.
+template <int L, int NQL, int THREADS>
 struct Inst {
-  static constexpr size_t kSmem = (size_t)NSMEM * NQ * THREADS * sizeof(double);
+  static constexpr size_t kSmem = (size_t)SL_COUNT * NQL * THREADS * sizeof(double);
   static cudaError_t configure(int* blocks_per_sm) {
-    cudaError_t e = cudaFuncSetAttribute(source_update_kernel<NQ, THREADS, NSMEM, false>,
+    cudaError_t e = cudaFuncSetAttribute(source_update_kernel<L, NQL, THREADS, false>,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem);
     if (e == cudaSuccess)
-      e = cudaFuncSetAttribute(source_update_kernel<NQ, THREADS, NSMEM, true>,
+      e = cudaFuncSetAttribute(source_update_kernel<L, NQL, THREADS, true>,
                                cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem);
     if (e == cudaSuccess)
-      e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, source_update_kernel<NQ, THREADS, NSMEM, false>,
+      e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, source_update_kernel<L, NQL, THREADS, false>,
                                                         THREADS, kSmem);
     return e;
   }
   static void launch(bool count, unsigned blocks, cudaStream_t st, const Params& P, const StatePtrs& S,
                      unsigned long long* stats, double* scratch) {
-    if (count) source_update_kernel<NQ, THREADS, NSMEM, true><<<blocks, THREADS, kSmem, st>>>(P, S, stats, scratch);
-    else source_update_kernel<NQ, THREADS, NSMEM, false><<<blocks, THREADS, kSmem, st>>>(P, S, stats, scratch);
+    if (count) source_update_kernel<L, NQL, THREADS, true><<<blocks, THREADS, kSmem, st>>>(P, S, stats, scratch);
+    else source_update_kernel<L, NQL, THREADS, false><<<blocks, THREADS, kSmem, st>>>(P, S, stats, scratch);
   }
 };
 
+// WHAT(L, NQL, THREADS); V = MGRHD_VARIANT (tuning experiments only; 0 = default)
 #define MGRHD_DISPATCH(Nq, V, WHAT)                            \
   do {                                                         \
-    if ((Nq) <= 4) { WHAT(4, 256, 6); }                        \
-    else if ((Nq) <= 8) { WHAT(8, 256, 6); }                   \
-    else if ((Nq) <= 16) { WHAT(16, 256, 6); }                 \
+    if ((Nq) <= 4) { WHAT(1, 5, 256); }                        \
+    else if ((Nq) <= 8) { WHAT(1, 9, 256); }                   \
+    else if ((Nq) <= 16) { WHAT(1, 17, 256); }                 \
     else if ((Nq) <= 32) {                                     \
-      if ((V) == 1) { WHAT(32, 192, 4); }                      \
-      else if ((V) == 2) { WHAT(32, 256, 3); }                 \
-      else if ((V) == 3) { WHAT(32, 384, 2); }                 \
-      else if ((V) == 4) { WHAT(32, 512, 0); }                 \
-      else { WHAT(32, 128, 6); }                               \
+      if ((V) == 1) { WHAT(1, 33, 128); }                      \
+      else if ((V) == 2) { WHAT(4, 9, 512); }                  \
+      else { WHAT(2, 17, 256); }                               \
     }                                                          \
-    else { WHAT(64, 64, 6); }                                  \
+    else {                                                     \
+      if ((V) == 1) { WHAT(2, 33, 128); }                      \
+      else { WHAT(4, 17, 256); }                               \
+    }                                                          \
   } while (0)
 
 // Fills ctx->cfg_* for ctx->P.Nq (called once by mgrhd_init).
@@ -192,7 +195,7 @@ static cudaError_t configure_ctx(mgrhd_ctx* ctx) {
   cudaError_t e = cudaSuccess;
   const char* ev = getenv("MGRHD_VARIANT");
   ctx->variant = ev ? atoi(ev) : 0;
-#define MGRHD_CFG(Q, T, M) e = Inst<Q, T, M>::configure(&ctx->cfg_bps); ctx->cfg_nq = Q; ctx->cfg_threads = T; ctx->cfg_nsmem = M
+#define MGRHD_CFG(LL, Q, T) e = Inst<LL, Q, T>::configure(&ctx->cfg_bps); ctx->cfg_l = LL; ctx->cfg_nq = Q; ctx->cfg_threads = T
   MGRHD_DISPATCH(ctx->P.Nq, ctx->variant, MGRHD_CFG);
 #undef MGRHD_CFG
   if (e == cudaSuccess && ctx->cfg_bps < 1) e = cudaErrorLaunchOutOfResources;
@@ -201,7 +204,7 @@ static cudaError_t configure_ctx(mgrhd_ctx* ctx) {
 
 // Bytes of lagged-flux scratch one launch needs at most: 3 * NQ doubles per resident thread.
 static size_t scratch_bytes(const mgrhd_ctx* ctx) {
-  return (size_t)(3 + SL_COUNT - ctx->cfg_nsmem) * ctx->cfg_nq * sizeof(double) * (size_t)ctx->sm_count * ctx->cfg_bps * ctx->cfg_threads;
+  return (size_t)3 * ctx->cfg_nq * sizeof(double) * (size_t)ctx->sm_count * ctx->cfg_bps * ctx->cfg_threads;
 }
 
 extern "C" {
@@ -290,10 +293,11 @@ static int launch_update(mgrhd_ctx* ctx, const StatePtrs& S, long long n, long l
   P.dt = dt; P.c = c; P.c_hat = chat; P.ncells = n; P.stride = stride;
   // persistent grid: one CTA per resident slot, fewer when the problem is small
   long long blocks = (long long)ctx->sm_count * ctx->cfg_bps;
-  const long long want = (n + ctx->cfg_threads - 1) / ctx->cfg_threads;
+  const long long cells_per_cta = ctx->cfg_threads / ctx->cfg_l;
+  const long long want = (n + cells_per_cta - 1) / cells_per_cta;
   if (blocks > want) blocks = want;
   const bool count = ctx->count_flops != 0;
-#define MGRHD_GO(Q, T, M) Inst<Q, T, M>::launch(count, (unsigned)blocks, st, P, S, ctx->d_stats, scratch)
+#define MGRHD_GO(LL, Q, T) Inst<LL, Q, T>::launch(count, (unsigned)blocks, st, P, S, ctx->d_stats, scratch)
   MGRHD_DISPATCH(P.Nq, ctx->variant, MGRHD_GO);
 #undef MGRHD_GO
   ctx->launches++;

@@ -35,6 +35,12 @@ __device__ __forceinline__ double fast_rcp(double x) {   // declared in mgrhd_pl
   return r;
 }
 
+// L1 prefetch of one global address (no register, no dependency)
+__device__ __forceinline__ void prefetch_l1(const double* p) {
+  asm volatile("prefetch.global.L1 [%0];" ::"l"(p));
+}
+constexpr int kPrefetchDist = 4;   // groups ahead
+
 __device__ __forceinline__ double norm3(double a, double b, double c) {
   return sqrt(fma(a, a, fma(b, b, c * c)));
 }
@@ -73,25 +79,38 @@ __device__ __forceinline__ void closure_vP(int closure, double E, double F0, dou
 // Lane phases of the flattened iteration.
 enum Phase : int { PH_LOAD = 0, PH_EVAL = 1, PH_FLUX = 2, PH_DONE = 3 };
 
-// Per-thread, per-group slots.  DA/DB/AG are reused for F_g^(new) between the two flux passes.
+// Per-lane, per-local-group shared-memory slots.  DA/DB/AG are reused for F_g^(new) between the
+// two flux passes.
 enum Slot : int { SL_R = 0, SL_DA, SL_DB, SL_VF, SL_AG, SL_CHIF, SL_COUNT };
 
-// NQ: compile-time group capacity (runtime Nq <= NQ); THREADS: CTA size; NSMEM: how many of the
-// SL_COUNT per-group slots live in shared memory (the rest go to the global scratch).
-// Dynamic shared memory: NSMEM * NQ * THREADS doubles.
-// scratch: (3 + SL_COUNT - NSMEM) * NQ * (gridDim.x*THREADS) doubles of global memory, private to
-// this launch: F_g^(t) of the cell in flight (the state's Frad holds the lagged F_g,k in place)
-// and the overflow slots.
+// Sum over the L lanes of a cell (butterfly: every lane ends with the same bits).
+template <int L>
+__device__ __forceinline__ double cell_sum(double v) {
+#pragma unroll
+  for (int off = 1; off < L; off <<= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
+  return v;
+}
+
+// L: lanes that share one cell (1, 2 or 4); lane `sub` of a cell owns edges e = i*L + sub and
+//    the groups g = e-1 below them, i = 0..NQL-1 ("steps"), so the L lanes of a cell evaluate
+//    NEIGHBOURING edges in the same step (x differs by r_g^(L-1) at most: same branch of
+//    planck_edge almost always) and the lower edge of a group comes from the lane to the left
+//    by one shuffle.  A warp works on 32/L cells at a time; per-thread state shrinks by L, so
+//    L times more threads fit beside the same shared memory.
+// NQL: steps per lane, NQL*L >= Nq+1.   THREADS: CTA size.
+// Dynamic shared memory: SL_COUNT * NQL * THREADS doubles, laid out [slot][step][thread].
+// scratch: 3 * NQL * (gridDim.x*THREADS) doubles of global memory, private to this launch:
+//    F_g^(t) of the cell in flight (the state's Frad holds the lagged F_g,k in place).
 //
-// One trip of the main loop, per warp (all loops over groups are entered warp-wide):
-//   LOAD  lanes without a cell take the next cells of the warp's chunk (scalars only);
-//   A     every lane with a cell evaluates all groups at its trial T (a1-a5); the Newton update
-//         of R_g decided in the previous trip is applied on the fly, the first evaluation of a
-//         cell also forms v.F_g and sum E_g, and a lane that has just finished a cell stores
-//         that cell's E_g here, so neither costs a loop of its own;
-//   B, C  lanes whose Newton iteration converged do the flux/momentum update and the outer test
+// One trip of the main loop, per warp (all loops over steps are entered warp-wide):
+//   LOAD  cells-slots without a cell take the next cells of the warp's chunk (scalars only);
+//   A     every lane with a cell evaluates its edges/groups at the trial T (a1-a5); the Newton
+//         update of R_g decided in the previous trip is applied on the fly, the first evaluation
+//         of a cell also forms v.F_g and sum E_g, and a lane that has just finished a cell
+//         stores that cell's E_g here, so none of these costs a loop of its own;
+//   B, C  cells whose Newton iteration converged do the flux/momentum update and the outer test
 //         (a6-a9); F_g is updated in place in the state, so a finished cell needs no flux store.
-template <int NQ, int THREADS, int NSMEM, bool COUNT>
+template <int L, int NQL, int THREADS, bool COUNT>
 __global__ void __launch_bounds__(THREADS, 1)
 source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ StatePtrs S,
                      unsigned long long* __restrict__ stats, double* __restrict__ scratch) {
@@ -101,7 +120,9 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
   __syncthreads();
 
   const int tid = threadIdx.x, lane = tid & 31;
+  const int sub = lane & (L - 1);                 // position of this lane within its cell
   const unsigned FULL = 0xffffffffu;
+  constexpr unsigned LEADERS = L == 1 ? 0xffffffffu : (L == 2 ? 0x55555555u : 0x11111111u);
   const int Nq = P.Nq;
   const long long n = P.ncells, stride = P.stride;
   const double dt = P.dt, c = P.c, chat = P.c_hat;
@@ -110,13 +131,9 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
 
   const long long tthreads = (long long)gridDim.x * THREADS;
   const long long gtid = (long long)blockIdx.x * THREADS + tid;
-  // slot s, group g of this thread: shared memory, or global scratch for the overflow slots
-  auto sm = [&](int s, int g) -> double& {
-    if (s < NSMEM) return smem[(s * NQ + g) * THREADS + tid];
-    return scratch[(long long)((3 + s - NSMEM) * NQ + g) * tthreads + gtid];
-  };
-  // F_g^(t), component i, of the cell in flight (global scratch, coalesced across the warp)
-  auto ft = [&](int i, int g) -> double& { return scratch[(long long)(i * NQ + g) * tthreads + gtid]; };
+  auto sm = [&](int s, int i) -> double& { return smem[(s * NQL + i) * THREADS + tid]; };
+  // F_g^(t), component k, step i of this lane (global scratch, coalesced across the warp)
+  auto ft = [&](int k, int i) -> double& { return scratch[(long long)(k * NQL + i) * tthreads + gtid]; };
 
   // this warp's contiguous chunk of cells [next, end)
   const long long nwarps = tthreads >> 5, wid = gtid >> 5;
@@ -129,7 +146,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
                cnt_den = 0, cnt_evals = 0, cnt_trips = 0, cnt_cells = 0;
   unsigned long long flops = 0;
 
-  // ---- per-lane cell state -----------------------------------------------------------------
+  // ---- per-cell state, replicated in the L lanes of the cell ------------------------------------
   int phase = PH_LOAD;
   long long cell = 0, fin_cell = -1;   // fin_cell: finished cell whose E_g store is still due
   double rho = 1.0, inv_rho = 1.0, chis = 1.0, inv_chis = 1.0, inv_Cv = 1.0, Egas_t = 0.0, Etot = 1.0;
@@ -138,27 +155,31 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
   bool first = false, pend = false;
   int it = 0, k = 0, evals = 0, trips = 0;
 
-  // a cell is finished: counters, scalar stores; its E_g store is done in the next loop A
+  // a cell is finished: counters and scalar stores by its first lane; E_g is stored in the next loop A
   auto finish = [&](double mn0, double mn1, double mn2, double Egas_new) {
     if (trips > 0) {
-      S.mom[0][cell] = mn0; S.mom[1][cell] = mn1; S.mom[2][cell] = mn2;
-      S.Egas[cell] = Egas_new;   // total gas energy; E_int = Egas - |mom|^2/(2 rho)
+      if (sub == 0) {
+        S.mom[0][cell] = mn0; S.mom[1][cell] = mn1; S.mom[2][cell] = mn2;
+        S.Egas[cell] = Egas_new;   // total gas energy; E_int = Egas - |mom|^2/(2 rho)
+      }
       fin_cell = cell;
     }
-    cnt_evals += evals;
-    cnt_trips += trips;
-    cnt_cells++;
-    atomicAdd(&s_hist[evals < MGRHD_HIST ? evals : MGRHD_HIST - 1], 1u);
-    atomicAdd(&s_hist[MGRHD_HIST + (trips < MGRHD_HIST ? trips : MGRHD_HIST - 1)], 1u);
+    if (sub == 0) {
+      cnt_evals += evals;
+      cnt_trips += trips;
+      cnt_cells++;
+      atomicAdd(&s_hist[evals < MGRHD_HIST ? evals : MGRHD_HIST - 1], 1u);
+      atomicAdd(&s_hist[MGRHD_HIST + (trips < MGRHD_HIST ? trips : MGRHD_HIST - 1)], 1u);
+    }
     phase = PH_LOAD;
   };
 
   while (true) {
     // ===== LOAD (a0): scalars of the next cell of the warp's chunk ================================
-    const unsigned need = __ballot_sync(FULL, phase == PH_LOAD);
+    const unsigned need = __ballot_sync(FULL, phase == PH_LOAD) & LEADERS;
     if (need) {
       if (phase == PH_LOAD) {
-        const long long cnew = next + __popc(need & ((1u << lane) - 1u));
+        const long long cnew = next + __popc(need & ((1u << (lane - sub)) - 1u));
         if (cnew < end) {
           cell = cnew;
           rho = S.rho[cell];
@@ -174,11 +195,11 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
           Ekin = (momk0 * momk0 + momk1 * momk1 + momk2 * momk2) * (0.5 * inv_rho);
           it = 0; k = 0; evals = 0; trips = 0;
           first = true; pend = false;
-          if (COUNT) flops += kFlopCell + kFlopCellGroup * Nq;
+          if (COUNT && sub == 0) flops += kFlopCell + kFlopCellGroup * Nq;
           if ((Egs - Ekin) * inv_Cv > 0.0) {
             phase = PH_EVAL;
           } else {                              // invalid state: count it, leave the cell as it is
-            cnt_Tnonpos++;
+            if (sub == 0) cnt_Tnonpos++;
             finish(0.0, 0.0, 0.0, 0.0);
           }
         } else {
@@ -189,7 +210,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
     }
     if (__all_sync(FULL, phase == PH_DONE)) break;
 
-    // ===== A: all groups at the trial temperature (a1-a5), then Eq. 49 ============================
+    // ===== A: all edges/groups at the trial temperature (a1-a5), then Eq. 49 =======================
     if (__any_sync(FULL, phase == PH_EVAL)) {
       const bool ev = phase == PH_EVAL;
       const bool fin = fin_cell >= 0;
@@ -203,45 +224,72 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
       const double guard_thr = 1e-280 * aT4;
       const double v0 = momk0 * inv_rho, v1 = momk1 * inv_rho, v2 = momk2 * inv_rho;
       double sumR = 0.0, sumAbsFR = 0.0, SFRq = 0.0, SJq = 0.0, sumEt = 0.0;
-      EdgeFn lo;
-      if (ev) {
-        lo = planck_edge(P.nu[0] * beta);
-        if (COUNT) flops += kFlopCellEval + lo.flops + (unsigned)(kFlopGroupEval * Nq);
-      }
-      // software prefetch of the next group's global operands
+      int eflops = 0;
+      EdgeFn prev;                                   // this lane's edge of the previous step
+      prev.yz = 0.0; prev.xi = 0.0; prev.small = true; prev.flops = 0;
+      const int src = sub == 0 ? lane + (L - 1) : lane - 1;   // lane that owns the lower edge
+      // register prefetch of the next step's global operands (group g = e - 1, e = i*L + sub)
       double nEt = 0.0, nF0 = 0.0, nF1 = 0.0, nF2 = 0.0, nEo = 0.0;
-      if (ev) nEt = S.Erad[cell];
-      if (ev && first) { nF0 = S.Frad[0][cell]; nF1 = S.Frad[1][cell]; nF2 = S.Frad[2][cell]; }
-      if (fin) nEo = S.Erad[fin_cell];
-      for (int g = 0; g < Nq; ++g) {
+      {
+        const int g0 = sub - 1;
+        if (g0 >= 0 && g0 < Nq) {
+          const long long o = (long long)g0 * stride;
+          if (ev) nEt = S.Erad[o + cell];
+          if (ev && first) { nF0 = S.Frad[0][o + cell]; nF1 = S.Frad[1][o + cell]; nF2 = S.Frad[2][o + cell]; }
+          if (fin) nEo = S.Erad[o + fin_cell];
+        }
+      }
+#pragma unroll 1
+      for (int i = 0; i < NQL; ++i) {
+        const int e = i * L + sub;                   // edge of this lane in this step
+        const int g = e - 1;                         // group below it
+        const bool vg = g >= 0 && g < Nq;
         const double Et = nEt, F0 = nF0, F1 = nF1, F2 = nF2, Eo = nEo;
-        if (g + 1 < Nq) {
-          const long long o1 = (long long)(g + 1) * stride;
-          if (ev) nEt = S.Erad[o1 + cell];
-          if (ev && first) { nF0 = S.Frad[0][o1 + cell]; nF1 = S.Frad[1][o1 + cell]; nF2 = S.Frad[2][o1 + cell]; }
-          if (fin) nEo = S.Erad[o1 + fin_cell];
+        {
+          const int g1 = g + L;
+          if (g1 >= 0 && g1 < Nq) {
+            const long long o1 = (long long)g1 * stride;
+            if (ev) nEt = S.Erad[o1 + cell];
+            if (ev && first) { nF0 = S.Frad[0][o1 + cell]; nF1 = S.Frad[1][o1 + cell]; nF2 = S.Frad[2][o1 + cell]; }
+            if (fin) nEo = S.Erad[o1 + fin_cell];
+          }
         }
         // a10 of the cell this lane finished in the previous trip: E_g^(t+1) = E_g^(t) + R_g
-        if (fin) S.Erad[(long long)g * stride + fin_cell] = Eo + sm(SL_R, g);
-        if (ev) {
-          // a1: edge functions at the upper edge of group g
-          const EdgeFn hi = planck_edge(P.nu[g + 1] * beta);
-          if (COUNT) flops += hi.flops;
+        if (fin && vg) S.Erad[(long long)g * stride + fin_cell] = Eo + sm(SL_R, i);
+        // a1: edge functions at this lane's edge; the lower edge of group g comes from the left
+        EdgeFn hi;
+        hi.yz = 0.0; hi.xi = 0.0; hi.small = false; hi.flops = 0;
+        if (ev && e <= Nq) hi = planck_edge(P.nu[e] * beta);
+        EdgeFn lo;
+        {
+          const bool last = sub == L - 1;
+          const double syz = last ? prev.yz : hi.yz, sxi = last ? prev.xi : hi.xi;
+          const int ssm = last ? (int)prev.small : (int)hi.small;
+          if (L == 1) { lo = prev; }
+          else {
+            lo.yz = __shfl_sync(FULL, syz, src);
+            lo.xi = __shfl_sync(FULL, sxi, src);
+            lo.small = __shfl_sync(FULL, ssm, src) != 0;
+          }
+        }
+        prev = hi;
+        if (COUNT) eflops += hi.flops;
+        if (ev && vg) {
           // R_g and the lagged v.F_g
           double R, vF;
           if (first) {
             R = 0.0;
             vF = fma(v0, F0, fma(v1, F1, v2 * F2));
             sumEt += Et;
-            sm(SL_R, g) = 0.0;
-            sm(SL_VF, g) = vF;
+            sm(SL_R, i) = 0.0;
+            sm(SL_VF, i) = vF;
           } else {
-            R = sm(SL_R, g);
+            R = sm(SL_R, i);
             if (pend) {     // Newton update decided at the end of the previous evaluation (Eq. 48)
-              R = fma(lam, sm(SL_DA, g), fma(ldx, sm(SL_DB, g), R));
-              sm(SL_R, g) = R;
+              R = fma(lam, sm(SL_DA, i), fma(ldx, sm(SL_DB, i), R));
+              sm(SL_R, i) = R;
             }
-            vF = sm(SL_VF, g);
+            vF = sm(SL_VF, i);
           }
           // a2: group Planck integral and Doppler boundary terms (Eq. 11, 18, 22)
           const double Bt = aT4 * planck_dY(lo, hi);
@@ -279,14 +327,18 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
           const double da = FR * q, db = fourBmDb * dBscale * q;
           SFRq += da;
           SJq += db;
-          sm(SL_DA, g) = da;
-          sm(SL_DB, g) = db;
-          sm(SL_AG, g) = fma(chiE, Bt, -Dthird);                   // chi_B Bt - D/3 (Eq. 51 source)
-          sm(SL_CHIF, g) = chiF;
-          lo = hi;
+          sm(SL_DA, i) = da;
+          sm(SL_DB, i) = db;
+          sm(SL_AG, i) = fma(chiE, Bt, -Dthird);                   // chi_B Bt - D/3 (Eq. 51 source)
+          sm(SL_CHIF, i) = chiF;
         }
       }
       fin_cell = fin ? -1 : fin_cell;
+      // the arrowhead reductions of Eq. 48 and the sums of Eq. 49-50 across the lanes of the cell
+      sumR = cell_sum<L>(sumR); sumAbsFR = cell_sum<L>(sumAbsFR);
+      SFRq = cell_sum<L>(SFRq); SJq = cell_sum<L>(SJq);
+      if (__any_sync(FULL, ev && first)) sumEt = cell_sum<L>(sumEt);
+      if (COUNT && ev) flops += (unsigned)eflops + (sub == 0 ? kFlopCellEval + kFlopGroupEval * Nq : 0);
       if (ev) {
         if (first) Etot = Egas_t + (chat / c) * sumEt;             // Eq. 50 as printed, S_g = 0
         first = false;
@@ -297,7 +349,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
         if (fabs(FG) * inv_Etot < P.newton_tol && c_over_chat * sumAbsFR * inv_Etot < P.newton_tol) {
           phase = PH_FLUX;                                          // Eq. 49 met
         } else if (it >= P.newton_maxit) {
-          cnt_newton_unconv++;
+          if (sub == 0) cnt_newton_unconv++;
           phase = PH_FLUX;
         } else {
           // Newton step: eliminate the gas row
@@ -306,13 +358,13 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
           lam = 1.0;
           for (int h = 0; h < 10 && !((Egs + lam * dx0 - Ekin) * inv_Cv > 0.0); ++h) {
             lam *= 0.5;
-            cnt_Tnonpos++;
+            if (sub == 0) cnt_Tnonpos++;
           }
           Egs += lam * dx0;
           ldx = lam * dx0;
           pend = true;          // R_g += lam da_g + ldx db_g, applied by the next evaluation
           it++;
-          if (COUNT) flops += kFlopStepCell + kFlopStepGroup * Nq;
+          if (COUNT && sub == 0) flops += kFlopStepCell + kFlopStepGroup * Nq;
         }
       }
     }
@@ -323,32 +375,39 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
       const bool t0 = trips == 0;       // first trip: F_g^(t) is still in the state, save it to the scratch
       const double v0 = momk0 * inv_rho, v1 = momk1 * inv_rho, v2 = momk2 * inv_rho;
       double sumR = 0.0, sumAbsR = 0.0, dF0 = 0.0, dF1 = 0.0, dF2 = 0.0;
-      bool rel_ok = true;
+      int rel_bad = 0;
       double nEt = 0.0, nFt0 = 0.0, nFt1 = 0.0, nFt2 = 0.0, nFk0 = 0.0, nFk1 = 0.0, nFk2 = 0.0;
-      if (fx) {
-        nEt = S.Erad[cell];
-        nFk0 = S.Frad[0][cell]; nFk1 = S.Frad[1][cell]; nFk2 = S.Frad[2][cell];
+      if (fx && sub >= 1 && sub - 1 < Nq) {
+        const long long o = (long long)(sub - 1) * stride + cell;
+        nEt = S.Erad[o];
+        nFk0 = S.Frad[0][o]; nFk1 = S.Frad[1][o]; nFk2 = S.Frad[2][o];
         if (!t0) { nFt0 = ft(0, 0); nFt1 = ft(1, 0); nFt2 = ft(2, 0); }
       }
-      for (int g = 0; g < Nq; ++g) {
+#pragma unroll 1
+      for (int i = 0; i < NQL; ++i) {
+        const int g = i * L + sub - 1;
+        const bool vg = fx && g >= 0 && g < Nq;
         const double Et = nEt, Fk0 = nFk0, Fk1 = nFk1, Fk2 = nFk2;
         const double Ft0 = t0 ? nFk0 : nFt0, Ft1 = t0 ? nFk1 : nFt1, Ft2 = t0 ? nFk2 : nFt2;
-        if (fx && g + 1 < Nq) {
-          const long long o1 = (long long)(g + 1) * stride + cell;
-          nEt = S.Erad[o1];
-          nFk0 = S.Frad[0][o1]; nFk1 = S.Frad[1][o1]; nFk2 = S.Frad[2][o1];
-          if (!t0) { nFt0 = ft(0, g + 1); nFt1 = ft(1, g + 1); nFt2 = ft(2, g + 1); }
+        {
+          const int g1 = g + L;
+          if (fx && g1 >= 0 && g1 < Nq) {
+            const long long o1 = (long long)g1 * stride + cell;
+            nEt = S.Erad[o1];
+            nFk0 = S.Frad[0][o1]; nFk1 = S.Frad[1][o1]; nFk2 = S.Frad[2][o1];
+            if (!t0) { nFt0 = ft(0, i + 1); nFt1 = ft(1, i + 1); nFt2 = ft(2, i + 1); }
+          }
         }
-        if (fx) {
+        if (vg) {
           const long long o = (long long)g * stride + cell;
-          const double R = sm(SL_R, g);
+          const double R = sm(SL_R, i);
           sumR += R;
           sumAbsR += fabs(R);
           const double Enew = Et + R;                               // E_g^(t+1) = E_g^(t) + R_g
           double p0, p1, p2;
           closure_vP(P.closure, Enew, Fk0, Fk1, Fk2, v0, v1, v2, c, p0, p1, p2);
           const double w = P.onepa[g] * (chis * P.k_mean[g]);       // (1 + alpha) chi_E
-          const double chiF = sm(SL_CHIF, g), A = sm(SL_AG, g);
+          const double chiF = sm(SL_CHIF, i), A = sm(SL_AG, i);
           const double dn = fma(cdt, chiF, 1.0);                    // 1 + c_hat chi_F dt > 0 (guarded in A)
           const double inv_dn = (dn > 1e-290 && dn < 1e290) ? fast_rcp(dn) : 1.0 / dn;
           const double Fn0 = fma(cdt, fma(v0, A, w * p0), Ft0) * inv_dn;
@@ -363,29 +422,39 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
             bool ok;
             if (f2 > 1e-280 && f2 < 1e280) ok = d2 <= rel2 * f2;
             else ok = norm3(e0, e1, e2) <= P.outer_rel_tol * norm3(Fn0, Fn1, Fn2);
-            if (!ok) rel_ok = false;
+            if (!ok) rel_bad = 1;
           }
-          if (t0) { ft(0, g) = Ft0; ft(1, g) = Ft1; ft(2, g) = Ft2; }
+          if (t0) { ft(0, i) = Ft0; ft(1, i) = Ft1; ft(2, i) = Ft2; }
           S.Frad[0][o] = Fn0; S.Frad[1][o] = Fn1; S.Frad[2][o] = Fn2;   // lagged flux of the next trip, in place
-          sm(SL_DA, g) = Fn0; sm(SL_DB, g) = Fn1; sm(SL_AG, g) = Fn2;   // kept on chip for loop C
+          sm(SL_DA, i) = Fn0; sm(SL_DB, i) = Fn1; sm(SL_AG, i) = Fn2;   // kept on chip for loop C
         }
       }
+      sumR = cell_sum<L>(sumR); sumAbsR = cell_sum<L>(sumAbsR);
+      dF0 = cell_sum<L>(dF0); dF1 = cell_sum<L>(dF1); dF2 = cell_sum<L>(dF2);
       double momn0 = 0.0, momn1 = 0.0, momn2 = 0.0, dW = 0.0;
       if (fx) {
         momn0 = momt0 - dF0 * icc; momn1 = momt1 - dF1 * icc; momn2 = momt2 - dF2 * icc;   // Eq. 52
         trips++;
-        if (COUNT) flops += kFlopOuterCell + kFlopOuterGroup * Nq;
+        if (COUNT && sub == 0) flops += kFlopOuterCell + kFlopOuterGroup * Nq;
       }
       const double vn0 = momn0 * inv_rho, vn1 = momn1 * inv_rho, vn2 = momn2 * inv_rho;
-      for (int g = 0; g < Nq; ++g) {
-        if (fx) {
-          const double vFn = fma(vn0, sm(SL_DA, g), fma(vn1, sm(SL_DB, g), vn2 * sm(SL_AG, g)));
-          const double wf = P.onepa[g] * sm(SL_CHIF, g) * inv_c;
-          dW += fabs(wf * (vFn - sm(SL_VF, g)));
-          sm(SL_VF, g) = vFn;                                       // lagged v.F_g of the next trip
+#pragma unroll 1
+      for (int i = 0; i < NQL; ++i) {
+        const int g = i * L + sub - 1;
+        if (fx && g >= 0 && g < Nq) {
+          const double vFn = fma(vn0, sm(SL_DA, i), fma(vn1, sm(SL_DB, i), vn2 * sm(SL_AG, i)));
+          const double wf = P.onepa[g] * sm(SL_CHIF, i) * inv_c;
+          dW += fabs(wf * (vFn - sm(SL_VF, i)));
+          sm(SL_VF, i) = vFn;                                       // lagged v.F_g of the next trip
         }
       }
+      dW = cell_sum<L>(dW);
+      if (L > 1) {
+#pragma unroll
+        for (int off = 1; off < L; off <<= 1) rel_bad |= __shfl_xor_sync(FULL, rel_bad, off);
+      }
       if (fx) {
+        bool rel_ok = rel_bad == 0;
         const double Egas_new = Egas_t - c_over_chat * sumR;
         if (P.outer_stop == 1) {
           const double d = norm3(momn0 - momk0, momn1 - momk1, momn2 - momk2);
@@ -395,7 +464,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
         if (delta <= P.outer_tol * fmax(sumAbsR, Etot) && rel_ok) {
           finish(momn0, momn1, momn2, Egas_new);
         } else if (k == P.outer_maxit - 1) {
-          cnt_outer_unconv++;
+          if (sub == 0) cnt_outer_unconv++;
           finish(momn0, momn1, momn2, Egas_new);
         } else {
           momk0 = momn0; momk1 = momn1; momk2 = momn2;
@@ -405,7 +474,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
           if ((Egs - Ekin) * inv_Cv > 0.0) {
             phase = PH_EVAL;
           } else {
-            cnt_Tnonpos++;
+            if (sub == 0) cnt_Tnonpos++;
             finish(momn0, momn1, momn2, Egas_new);
           }
         }
@@ -415,9 +484,12 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
 
   // E_g store of the last cell of each lane (no further loop A ran for it)
   if (fin_cell >= 0)
-    for (int g = 0; g < Nq; ++g) {
-      const long long o = (long long)g * stride + fin_cell;
-      S.Erad[o] = S.Erad[o] + sm(SL_R, g);
+    for (int i = 0; i < NQL; ++i) {
+      const int g = i * L + sub - 1;
+      if (g >= 0 && g < Nq) {
+        const long long o = (long long)g * stride + fin_cell;
+        S.Erad[o] = S.Erad[o] + sm(SL_R, i);
+      }
     }
 
   // ---- diagnostics: warp-reduce the scalar counters, one atomic per warp ------------------
