@@ -94,19 +94,21 @@ void cheb_fit_monomial(long double (*f)(long double), long double a, long double
 void fill_planck_tables(PlanckTables& t) {
   for (int n = 1; n <= kSmallTerms; ++n) {
     const long double b = bern_over_fact(n);
-    t.xi_c[n - 1] = (double)b;
-    t.y_c[n - 1] = (double)(b / (2.0L * n + 3.0L));
+    t.sp[n - 1].a = (double)(b / (2.0L * n + 3.0L));
+    t.sp[n - 1].b = (double)b;
   }
-  cheb_fit_monomial(Z_host, kXS, kXL, 48, kMidTerms, t.mz);
-  cheb_fit_monomial(Xi_host, kXS, kXL, 48, kMidTerms, t.mx);
+  double mz[kMidTerms], mx[kMidTerms];
+  cheb_fit_monomial(Z_host, kXS, kXL, 48, kMidTerms, mz);
+  cheb_fit_monomial(Xi_host, kXS, kXL, 48, kMidTerms, mx);
+  for (int k = 0; k < kMidTerms; ++k) { t.mp[k].a = mz[k]; t.mp[k].b = mx[k]; }
   t.mid_s = (double)(2.0L / ((long double)kXL - (long double)kXS));
   t.mid_o = (double)(-((long double)kXL + (long double)kXS) / ((long double)kXL - (long double)kXS));
   for (int n = 1; n <= kLargeTerms; ++n) {
     const long double q = 1.0L / n;
-    t.l3[n - 1] = (double)(kC15Pi4L * q);
-    t.l2[n - 1] = (double)(3.0L * kC15Pi4L * q * q);
-    t.l1[n - 1] = (double)(6.0L * kC15Pi4L * q * q * q);
-    t.l0[n - 1] = (double)(6.0L * kC15Pi4L * q * q * q * q);
+    t.l32[n - 1].a = (double)(kC15Pi4L * q);
+    t.l32[n - 1].b = (double)(3.0L * kC15Pi4L * q * q);
+    t.l10[n - 1].a = (double)(6.0L * kC15Pi4L * q * q * q);
+    t.l10[n - 1].b = (double)(6.0L * kC15Pi4L * q * q * q * q);
   }
 }
 
@@ -119,9 +121,10 @@ cudaError_t upload_tables_for_current_device() {
   if (e != cudaSuccess) return e;
   if (dev < 0 || dev >= 16) return cudaErrorInvalidDevice;
   std::call_once(g_tables_once[dev], [dev]() {
-    PlanckTables t;
-    fill_planck_tables(t);
-    g_tables_err[dev] = cudaMemcpyToSymbol(c_planck, &t, sizeof t);
+    static PlanckTables t[2];
+    fill_planck_tables(t[0]);
+    t[1] = t[0];
+    g_tables_err[dev] = cudaMemcpyToSymbol(mgrhd_c_planck, t, sizeof t);
   });
   return g_tables_err[dev];
 }
@@ -180,9 +183,9 @@ struct Inst {
     else if ((Nq) <= 8) { WHAT(1, 9, 256); }                   \
     else if ((Nq) <= 16) { WHAT(1, 17, 256); }                 \
     else if ((Nq) <= 32) {                                     \
-      if ((V) == 1) { WHAT(1, 33, 128); }                      \
+      if ((V) == 1) { WHAT(2, 17, 256); }                      \
       else if ((V) == 2) { WHAT(4, 9, 512); }                  \
-      else { WHAT(2, 17, 256); }                               \
+      else { WHAT(4, 9, 384); }                                \
     }                                                          \
     else {                                                     \
       if ((V) == 1) { WHAT(2, 33, 128); }                      \

@@ -259,7 +259,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
         // a1: edge functions at this lane's edge; the lower edge of group g comes from the left
         EdgeFn hi;
         hi.yz = 0.0; hi.xi = 0.0; hi.small = false; hi.flops = 0;
-        if (ev && e <= Nq) hi = planck_edge(P.nu[e] * beta);
+        if (ev && e <= Nq) hi = planck_edge(P.nu[e] * beta, planck_table_base(i));
         EdgeFn lo;
         {
           const bool last = sub == L - 1;
@@ -536,7 +536,7 @@ __global__ void planck_edge_kernel(const double* __restrict__ x, long long n, do
                                    double* __restrict__ xi, int* __restrict__ is_y) {
   for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n;
        i += (long long)gridDim.x * blockDim.x) {
-    const EdgeFn e = planck_edge(x[i]);
+    const EdgeFn e = planck_edge(x[i], planck_table_base((int)(i & 1)));
     yz[i] = e.yz;
     xi[i] = e.xi;
     is_y[i] = e.small ? 1 : 0;

@@ -84,16 +84,19 @@ constexpr int kMidTerms = 24;     // monomial terms of the mid-range fits, kXS <
 constexpr int kLargeTerms = 7;    // terms of the e^{-nx} series, x >= kXL
 constexpr double kXS = 1.25;
 constexpr double kXL = 5.5;
-struct PlanckTables {
+// Coefficients are stored in PAIRS (one 16-byte constant load feeds both Horner chains).
+struct Pair { double a, b; };
+struct alignas(16) PlanckTables {
   // t/(e^t-1) = 1 - t/2 + sum_{n>=1} b_{2n} t^(2n),  b_{2n} = B_{2n}/(2n)!
-  double xi_c[kSmallTerms];   // b_{2n}          : Xi(x) = C x^3 (1 - x/2 + sum xi_c[n-1] x^(2n))
-  double y_c[kSmallTerms];    // b_{2n}/(2n+3)   : Y(x)  = C x^3 (1/3 - x/8 + sum y_c[n-1] x^(2n))
-  // mid range: Z(x) = sum mz[k] t^k, Xi(x) = sum mx[k] t^k, t = mid_s * x + mid_o in [-1, 1]
-  double mz[kMidTerms];
-  double mx[kMidTerms];
-  double mid_s, mid_o;
+  //   sp[n-1] = { b_{2n}/(2n+3), b_{2n} } :  Y(x)  = C x^3 (1/3 - x/8 + sum sp[n-1].a x^(2n)),
+  //                                          Xi(x) = C x^3 (1 - x/2 + sum sp[n-1].b x^(2n))
+  Pair sp[kSmallTerms];
+  // mid range: Z(x) = sum mp[k].a t^k, Xi(x) = sum mp[k].b t^k, t = mid_s * x + mid_o in [-1, 1]
+  Pair mp[kMidTerms];
   // large x: Z(x) = C sum_{n=1..kLargeTerms} e^{-nx} (x^3/n + 3x^2/n^2 + 6x/n^3 + 6/n^4)
-  double l3[kLargeTerms], l2[kLargeTerms], l1[kLargeTerms], l0[kLargeTerms];   // C/n, 3C/n^2, 6C/n^3, 6C/n^4
+  Pair l32[kLargeTerms];      // { C/n, 3C/n^2 }
+  Pair l10[kLargeTerms];      // { 6C/n^3, 6C/n^4 }
+  double mid_s, mid_o;
 };
 
 }  // namespace mgrhd

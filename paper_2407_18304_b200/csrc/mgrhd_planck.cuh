@@ -18,13 +18,56 @@
 #pragma once
 #include "mgrhd_params.h"
 
-namespace mgrhd {
+// The tables live outside the namespace with C linkage so inline PTX can name the symbol.
+// TWO identical copies: the step loop addresses copy (step & 1), see TableBase below.
+extern "C" {
+__constant__ mgrhd::PlanckTables mgrhd_c_planck[2];
+}
 
-__constant__ PlanckTables c_planck;
+namespace mgrhd {
 
 constexpr double kC15Pi4 = 0.15398973382026503;       // 15/pi^4
 
 __device__ __forceinline__ double fast_rcp(double x);  // mgrhd_kernels.cuh
+
+// Address (in the .const space) of one copy of the tables.  The caller derives `which` from the
+// step counter of its loop: DFMA has no constant-bank operand form on sm_100, so a coefficient
+// must be loaded into a (uniform) register either way, and when the table address is loop
+// invariant ptxas hoists ALL ~100 coefficients of ALL branches ahead of the step loop, runs out
+// of uniform registers and shuffles them through spills inside the loop (2-3 extra instructions
+// per coefficient).  A base that changes with the step keeps each 16-byte load (two
+// coefficients, one per Horner chain) next to its use.
+struct TableBase { unsigned long long addr; };
+__device__ __forceinline__ TableBase planck_table_base(int which) {
+  unsigned long long a;
+  asm("mov.u64 %0, mgrhd_c_planck;" : "=l"(a));
+  TableBase t;
+  t.addr = a + (unsigned long long)(which & 1) * sizeof(PlanckTables);
+  return t;
+}
+
+template <int OFF>
+__device__ __forceinline__ void ldc_pair(TableBase tb, double& a, double& b) {
+  asm("ld.const.v2.f64 {%0, %1}, [%2+%3];" : "=d"(a), "=d"(b) : "l"(tb.addr), "n"(OFF));
+}
+
+// Two Horner chains sharing their coefficient loads: (sa, sb) <- (sa, sb) * t + table[N-1..0]
+template <int BASE, int N>
+__device__ __forceinline__ void horner_pair(TableBase tb, double t, double& sa, double& sb) {
+  if constexpr (N > 0) {
+    double ca, cb;
+    ldc_pair<BASE + 16 * (N - 1)>(tb, ca, cb);
+    sa = fma(sa, t, ca);
+    sb = fma(sb, t, cb);
+    horner_pair<BASE, N - 1>(tb, t, sa, sb);
+  }
+}
+
+constexpr int kOffSp = 0;
+constexpr int kOffMp = kOffSp + 16 * kSmallTerms;
+constexpr int kOffL32 = kOffMp + 16 * kMidTerms;
+constexpr int kOffL10 = kOffL32 + 16 * kLargeTerms;
+constexpr int kOffMid = kOffL10 + 16 * kLargeTerms;
 
 struct EdgeFn {
   double yz;   // Y(x) if small, else Z(x)
@@ -33,18 +76,27 @@ struct EdgeFn {
   int flops;   // algorithmic flop count of this evaluation (dead code unless counted)
 };
 
+// e^{-n x} series term n (1-based) folded into sum: sum <- sum*u + (l3 x^3 + l2 x^2 + l1 x + l0)
+template <int N>
+__device__ __forceinline__ void large_terms(TableBase tb, double x, double u, double& sum) {
+  if constexpr (N > 0) {
+    double c3, c2, c1, c0;
+    ldc_pair<kOffL32 + 16 * (N - 1)>(tb, c3, c2);
+    ldc_pair<kOffL10 + 16 * (N - 1)>(tb, c1, c0);
+    const double pn = fma(fma(fma(c3, x, c2), x, c1), x, c0);
+    sum = fma(sum, u, pn);
+    large_terms<N - 1>(tb, x, u, sum);
+  }
+}
+
 // x in [0, +inf].  x == 0 -> (Y=0, Xi=0); x == +inf or e^-x == 0 -> (Z=0, Xi=0).
-__device__ __forceinline__ EdgeFn planck_edge(double x) {
+__device__ __forceinline__ EdgeFn planck_edge(double x, TableBase tb) {
   EdgeFn r;
   if (x < kXS) {
     const double x2 = x * x;
-    double sy = c_planck.y_c[kSmallTerms - 1];
-    double sx = c_planck.xi_c[kSmallTerms - 1];
-#pragma unroll
-    for (int n = kSmallTerms - 2; n >= 0; --n) {
-      sy = fma(sy, x2, c_planck.y_c[n]);
-      sx = fma(sx, x2, c_planck.xi_c[n]);
-    }
+    double sy, sx;
+    ldc_pair<kOffSp + 16 * (kSmallTerms - 1)>(tb, sy, sx);
+    horner_pair<kOffSp, kSmallTerms - 1>(tb, x2, sy, sx);
     const double x3 = x2 * x;
     // Y = C x^3 (1/3 - x/8 + x^2 sy),  Xi = C x^3 (1 - x/2 + x^2 sx)
     r.yz = kC15Pi4 * x3 * fma(x2, sy, fma(-0.125, x, 1.0 / 3.0));
@@ -55,14 +107,12 @@ __device__ __forceinline__ EdgeFn planck_edge(double x) {
   }
   r.small = false;
   if (x < kXL) {
-    const double t = fma(x, c_planck.mid_s, c_planck.mid_o);
-    double sz = c_planck.mz[kMidTerms - 1];
-    double sx = c_planck.mx[kMidTerms - 1];
-#pragma unroll
-    for (int n = kMidTerms - 2; n >= 0; --n) {
-      sz = fma(sz, t, c_planck.mz[n]);
-      sx = fma(sx, t, c_planck.mx[n]);
-    }
+    double ms, mo;
+    ldc_pair<kOffMid>(tb, ms, mo);
+    const double t = fma(x, ms, mo);
+    double sz, sx;
+    ldc_pair<kOffMp + 16 * (kMidTerms - 1)>(tb, sz, sx);
+    horner_pair<kOffMp, kMidTerms - 1>(tb, t, sz, sx);
     r.yz = sz;
     r.xi = sx;
     r.flops = kFlopEdgeMid;
@@ -77,11 +127,7 @@ __device__ __forceinline__ EdgeFn planck_edge(double x) {
   }
   const double x2 = x * x;
   double sum = 0.0;
-#pragma unroll
-  for (int n = kLargeTerms - 1; n >= 0; --n) {
-    const double pn = fma(fma(fma(c_planck.l3[n], x, c_planck.l2[n]), x, c_planck.l1[n]), x, c_planck.l0[n]);
-    sum = fma(sum, u, pn);
-  }
+  large_terms<kLargeTerms>(tb, x, u, sum);
   r.yz = sum * u;
   r.xi = kC15Pi4 * (x2 * x2) * (u * fast_rcp(1.0 - u));
   r.flops = kFlopEdgeLarge;
