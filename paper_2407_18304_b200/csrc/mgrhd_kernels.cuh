@@ -225,9 +225,11 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
       const double v0 = momk0 * inv_rho, v1 = momk1 * inv_rho, v2 = momk2 * inv_rho;
       double sumR = 0.0, sumAbsFR = 0.0, SFRq = 0.0, SJq = 0.0, sumEt = 0.0;
       int eflops = 0;
-      EdgeFn prev;                                   // this lane's edge of the previous step
-      prev.yz = 0.0; prev.xi = 0.0; prev.small = true; prev.flops = 0;
+      double prev_yz = 0.0, prev_xi = 0.0;           // this lane's edge of the previous step
+      int prev_small = 1;
       const int src = sub == 0 ? lane + (L - 1) : lane - 1;   // lane that owns the lower edge
+      const bool last = sub == L - 1;
+      const bool evf = ev && first, evp = ev && pend;
       // register prefetch of the next step's global operands (group g = e - 1, e = i*L + sub)
       double nEt = 0.0, nF0 = 0.0, nF1 = 0.0, nF2 = 0.0, nEo = 0.0;
       {
@@ -235,101 +237,92 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
         if (g0 >= 0 && g0 < Nq) {
           const long long o = (long long)g0 * stride;
           if (ev) nEt = S.Erad[o + cell];
-          if (ev && first) { nF0 = S.Frad[0][o + cell]; nF1 = S.Frad[1][o + cell]; nF2 = S.Frad[2][o + cell]; }
+          if (evf) { nF0 = S.Frad[0][o + cell]; nF1 = S.Frad[1][o + cell]; nF2 = S.Frad[2][o + cell]; }
           if (fin) nEo = S.Erad[o + fin_cell];
         }
       }
+      // The body below is executed by ALL lanes of the warp with per-lane predicates (a lane
+      // without a cell or without a group in this step computes on harmless values and stores
+      // nothing): no divergent branches, so the compiler needs no reconvergence code.
 #pragma unroll 1
       for (int i = 0; i < NQL; ++i) {
         const int e = i * L + sub;                   // edge of this lane in this step
         const int g = e - 1;                         // group below it
         const bool vg = g >= 0 && g < Nq;
+        const bool evg = ev && vg;
+        const int gi = vg ? g : 0;                   // safe table index
         const double Et = nEt, F0 = nF0, F1 = nF1, F2 = nF2, Eo = nEo;
         {
           const int g1 = g + L;
           if (g1 >= 0 && g1 < Nq) {
             const long long o1 = (long long)g1 * stride;
             if (ev) nEt = S.Erad[o1 + cell];
-            if (ev && first) { nF0 = S.Frad[0][o1 + cell]; nF1 = S.Frad[1][o1 + cell]; nF2 = S.Frad[2][o1 + cell]; }
+            if (evf) { nF0 = S.Frad[0][o1 + cell]; nF1 = S.Frad[1][o1 + cell]; nF2 = S.Frad[2][o1 + cell]; }
             if (fin) nEo = S.Erad[o1 + fin_cell];
           }
         }
+        const double Rold = sm(SL_R, i);
         // a10 of the cell this lane finished in the previous trip: E_g^(t+1) = E_g^(t) + R_g
-        if (fin && vg) S.Erad[(long long)g * stride + fin_cell] = Eo + sm(SL_R, i);
+        if (fin && vg) S.Erad[(long long)g * stride + fin_cell] = Eo + Rold;
         // a1: edge functions at this lane's edge; the lower edge of group g comes from the left
-        EdgeFn hi;
-        hi.yz = 0.0; hi.xi = 0.0; hi.small = false; hi.flops = 0;
-        if (ev && e <= Nq) hi = planck_edge(P.nu[e] * beta, planck_table_base(i));
-        EdgeFn lo;
-        {
-          const bool last = sub == L - 1;
-          const double syz = last ? prev.yz : hi.yz, sxi = last ? prev.xi : hi.xi;
-          const int ssm = last ? (int)prev.small : (int)hi.small;
-          if (L == 1) { lo = prev; }
-          else {
-            lo.yz = __shfl_sync(FULL, syz, src);
-            lo.xi = __shfl_sync(FULL, sxi, src);
-            lo.small = __shfl_sync(FULL, ssm, src) != 0;
-          }
+        double hi_yz, hi_xi;
+        bool hi_small;
+        int hf;
+        planck_edge_w(ev && e <= Nq ? P.nu[e <= Nq ? e : Nq] * beta : __longlong_as_double(0x7ff8000000000000ll),
+                      i, hi_yz, hi_xi, hi_small, hf);
+        if (COUNT) eflops += hf;
+        double lo_yz, lo_xi;
+        bool lo_small;
+        if (L == 1) {
+          lo_yz = prev_yz; lo_xi = prev_xi; lo_small = prev_small != 0;
+        } else {
+          lo_yz = __shfl_sync(FULL, last ? prev_yz : hi_yz, src);
+          lo_xi = __shfl_sync(FULL, last ? prev_xi : hi_xi, src);
+          lo_small = __shfl_sync(FULL, last ? prev_small : (int)hi_small, src) != 0;
         }
-        prev = hi;
-        if (COUNT) eflops += hi.flops;
-        if (ev && vg) {
-          // R_g and the lagged v.F_g
-          double R, vF;
-          if (first) {
-            R = 0.0;
-            vF = fma(v0, F0, fma(v1, F1, v2 * F2));
-            sumEt += Et;
-            sm(SL_R, i) = 0.0;
-            sm(SL_VF, i) = vF;
-          } else {
-            R = sm(SL_R, i);
-            if (pend) {     // Newton update decided at the end of the previous evaluation (Eq. 48)
-              R = fma(lam, sm(SL_DA, i), fma(ldx, sm(SL_DB, i), R));
-              sm(SL_R, i) = R;
-            }
-            vF = sm(SL_VF, i);
-          }
-          // a2: group Planck integral and Doppler boundary terms (Eq. 11, 18, 22)
-          const double Bt = aT4 * planck_dY(lo, hi);
-          const double Db = aT4 * (hi.xi - lo.xi);
-          const double D = aT4 * chis * fma(P.k_hi[g], hi.xi, -P.k_lo[g] * lo.xi);
-          const double chiE = chis * P.k_mean[g];                  // = chi_B (alpha_Q = -1 for both)
-          const double fourBmDb = fma(4.0, Bt, -Db);               // 3 x denominator of Eq. 27 = T dBt/dT
-          // a3: flux-mean opacity, Eq. 27, with the Wien-limit guard (S8)
-          const double den = fourBmDb * (1.0 / 3.0);
-          const double Dthird = D * (1.0 / 3.0);
-          const double num = fma(chis * Bt, P.k_num[g], -Dthird);  // (chi_B + chi_E/3 + alpha chi_E/3) Bt - D/3
-          double chiF;
-          if (!(den >= guard_thr) || isinf(den)) {
-            chiF = chis * P.k_lo[g];
-            if (evals == 0) cnt_guard++;
-          } else if (den > 1e-290 && den < 1e290) {
-            chiF = num * fast_rcp(den);
-          } else {
-            chiF = num / den;
-          }
-          if (!(fma(cdt, chiF, 1.0) > 0.0)) {
-            if (evals == 0) cnt_den++;
-            chiF = chiE;
-          }
-          // a4: residuals (Eq. 41; Eq. 42 solved for E_g)
-          const double inv_chiE = inv_chis * P.inv_k_mean[g];
-          const double itau = itau_c * P.inv_k_mean[g];
-          const double W = P.onepa[g] * chiF * vF * inv_c;
-          const double Eg = fma(W * inv_chiE, inv_c, Bt) - R * itau;
-          const double FR = Eg - Et - R;
+        prev_yz = hi_yz; prev_xi = hi_xi; prev_small = hi_small;
+        // R_g (Newton update decided at the end of the previous evaluation, Eq. 48) and lagged v.F_g
+        double R = evp ? fma(lam, sm(SL_DA, i), fma(ldx, sm(SL_DB, i), Rold)) : Rold;
+        double vF = sm(SL_VF, i);
+        if (first) { R = 0.0; vF = fma(v0, F0, fma(v1, F1, v2 * F2)); }
+        if (evg) { sm(SL_R, i) = R; sm(SL_VF, i) = vF; }
+        if (evf && vg) sumEt += Et;
+        // a2: group Planck integral and Doppler boundary terms (Eq. 11, 18, 22)
+        const double dY = hi_small ? hi_yz - lo_yz : (lo_small ? (1.0 - lo_yz) - hi_yz : lo_yz - hi_yz);
+        const double Bt = aT4 * dY;
+        const double Db = aT4 * (hi_xi - lo_xi);
+        const double D = aT4 * chis * fma(P.k_hi[gi], hi_xi, -P.k_lo[gi] * lo_xi);
+        const double chiE = chis * P.k_mean[gi];                 // = chi_B (alpha_Q = -1 for both)
+        const double fourBmDb = fma(4.0, Bt, -Db);               // 3 x denominator of Eq. 27 = T dBt/dT
+        // a3: flux-mean opacity, Eq. 27, with the Wien-limit guard (S8)
+        const double den = fourBmDb * (1.0 / 3.0);
+        const double Dthird = D * (1.0 / 3.0);
+        const double num = fma(chis * Bt, P.k_num[gi], -Dthird); // (chi_B + chi_E/3 + alpha chi_E/3) Bt - D/3
+        const bool guard = !(den >= guard_thr) || isinf(den);
+        const bool den_normal = den > 1e-290 && den < 1e290;
+        double chiF = num * fast_rcp(den_normal ? den : 1.0);
+        if (__any_sync(FULL, evg && !guard && !den_normal)) chiF = den_normal ? chiF : num / den;   // rare: IEEE division
+        if (guard) chiF = chis * P.k_lo[gi];
+        const bool denbad = !(fma(cdt, chiF, 1.0) > 0.0);
+        if (denbad) chiF = chiE;
+        if (evg && evals == 0) { cnt_guard += guard ? 1u : 0u; cnt_den += denbad ? 1u : 0u; }
+        // a4: residuals (Eq. 41; Eq. 42 solved for E_g)
+        const double inv_chiE = inv_chis * P.inv_k_mean[gi];
+        const double itau = itau_c * P.inv_k_mean[gi];
+        const double W = P.onepa[gi] * chiF * vF * inv_c;
+        const double Eg = fma(W * inv_chiE, inv_c, Bt) - R * itau;
+        const double FR = Eg - Et - R;
+        // a5: Jacobian (Eq. 44-47) folded into the arrowhead elimination (Eq. 48): 1/J_gg = -q
+        const double q = fast_rcp(1.0 + itau);
+        const double da = FR * q, db = fourBmDb * dBscale * q;
+        if (evg) {
           sumR += R;
           sumAbsFR += fabs(FR);
-          // a5: Jacobian (Eq. 44-47) folded into the arrowhead elimination (Eq. 48): 1/J_gg = -q
-          const double q = fast_rcp(1.0 + itau);
-          const double da = FR * q, db = fourBmDb * dBscale * q;
           SFRq += da;
           SJq += db;
           sm(SL_DA, i) = da;
           sm(SL_DB, i) = db;
-          sm(SL_AG, i) = fma(chiE, Bt, -Dthird);                   // chi_B Bt - D/3 (Eq. 51 source)
+          sm(SL_AG, i) = fma(chiE, Bt, -Dthird);                 // chi_B Bt - D/3 (Eq. 51 source)
           sm(SL_CHIF, i) = chiF;
         }
       }

@@ -134,6 +134,65 @@ __device__ __forceinline__ EdgeFn planck_edge(double x, TableBase tb) {
   return r;
 }
 
+// The same three branches for a CONVERGED warp: every branch that any lane needs is executed by
+// all 32 lanes (a divergent branch costs the warp the same issue slots) and the result is kept by
+// the lanes it belongs to.  Converged code lets the coefficient loads run on the uniform
+// datapath, two coefficients per load, with no reconvergence bookkeeping.  `which` must be
+// warp-uniform and change with the caller's loop counter (see TableBase above).
+// x = NaN marks a lane without an edge: it matches no branch and gets (0, 0, large).
+__device__ __forceinline__ void planck_edge_w(double x, int which, double& yz, double& xi, bool& small,
+                                              int& flops) {
+  const PlanckTables& tb = mgrhd_c_planck[which & 1];
+  const unsigned FULL = 0xffffffffu;
+  const bool inS = x < kXS;
+  const bool inM = x >= kXS && x < kXL;
+  const bool inL = x >= kXL;
+  yz = 0.0; xi = 0.0; small = inS; flops = 0;
+  if (__any_sync(FULL, inS)) {
+    const double x2 = x * x;
+    double sy = tb.sp[kSmallTerms - 1].a, sx = tb.sp[kSmallTerms - 1].b;
+#pragma unroll
+    for (int n = kSmallTerms - 2; n >= 0; --n) {
+      sy = fma(sy, x2, tb.sp[n].a);
+      sx = fma(sx, x2, tb.sp[n].b);
+    }
+    const double cx3 = kC15Pi4 * (x2 * x);
+    // Y = C x^3 (1/3 - x/8 + x^2 sy),  Xi = C x^3 (1 - x/2 + x^2 sx)
+    const double y = cx3 * fma(x2, sy, fma(-0.125, x, 1.0 / 3.0));
+    const double z = cx3 * fma(x2, sx, fma(-0.5, x, 1.0));
+    if (inS) { yz = y; xi = z; flops = kFlopEdgeSmall; }
+  }
+  if (__any_sync(FULL, inM)) {
+    const double t = fma(x, tb.mid_s, tb.mid_o);
+    double sz = tb.mp[kMidTerms - 1].a, sx = tb.mp[kMidTerms - 1].b;
+#pragma unroll
+    for (int n = kMidTerms - 2; n >= 0; --n) {
+      sz = fma(sz, t, tb.mp[n].a);
+      sx = fma(sx, t, tb.mp[n].b);
+    }
+    if (inM) { yz = sz; xi = sx; flops = kFlopEdgeMid; }
+  }
+  if (__any_sync(FULL, inL)) {
+    const double u = exp(-x);            // 0 on underflow and for x = +inf
+    const double xx = inL && u > 0.0 ? x : 1.0;   // keeps inf * 0 out of the polynomials
+    double sum = 0.0;
+#pragma unroll
+    for (int n = kLargeTerms - 1; n >= 0; --n) {
+      const double pn = fma(fma(fma(tb.l32[n].a, xx, tb.l32[n].b), xx, tb.l10[n].a), xx, tb.l10[n].b);
+      sum = fma(sum, u, pn);
+    }
+    const double x2 = xx * xx;
+    const double z = sum * u;
+    const double w = kC15Pi4 * (x2 * x2) * (u * fast_rcp(1.0 - u));
+    if (inL) {
+      const bool live = u > 0.0;
+      yz = live ? z : 0.0;
+      xi = live ? w : 0.0;
+      flops = live ? kFlopEdgeLarge : kFlopEdgeZero;
+    }
+  }
+}
+
 // Y(hi) - Y(lo) for two edges of one group (lo below hi).
 __device__ __forceinline__ double planck_dY(const EdgeFn& lo, const EdgeFn& hi) {
   if (hi.small) return hi.yz - lo.yz;          // both small
