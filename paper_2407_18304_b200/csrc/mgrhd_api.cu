@@ -185,6 +185,8 @@ struct Inst {
     else if ((Nq) <= 32) {                                     \
       if ((V) == 1) { WHAT(2, 17, 256); }                      \
       else if ((V) == 2) { WHAT(4, 9, 512); }                  \
+      else if ((V) == 3) { WHAT(4, 9, 416); }                  \
+      else if ((V) == 4) { WHAT(4, 9, 448); }                  \
       else { WHAT(4, 9, 384); }                                \
     }                                                          \
     else {                                                     \

@@ -46,34 +46,30 @@ __device__ __forceinline__ double norm3(double a, double b, double c) {
 }
 
 // v^j P^{ji} for one group (closure reading S7 of DESIGN.md): Levermore/M1
-// or Eddington P = E/3 I.
-__device__ __forceinline__ void closure_vP(int closure, double E, double F0, double F1, double F2,
+// or Eddington P = E/3 I.  Branch-free for a converged warp: with t = F/(cE),
+// f^2 = |t|^2 and n (n.v) = t (t.v)/f^2, so neither |F| nor a unit vector is formed.
+// `live` marks lanes whose result is used (the others may hold anything).
+__device__ __forceinline__ void closure_vP(int closure, bool live, double E, double F0, double F1, double F2,
                                            double v0, double v1, double v2, double c,
                                            double& p0, double& p1, double& p2) {
-  const double Fn = norm3(F0, F1, F2);
-  if (closure == 1 || !(E > 0.0) || Fn == 0.0) {
-    const double t = E * (1.0 / 3.0);
-    p0 = t * v0; p1 = t * v1; p2 = t * v2;
-    return;
-  }
   const double cE = c * E;
-  double f, inv_Fn;
-  if (cE > 1e-290 && cE < 1e290 && Fn > 1e-290 && Fn < 1e290) {
-    f = Fn * fast_rcp(cE);
-    inv_Fn = fast_rcp(Fn);
-  } else {               // denormal / huge group energies: IEEE division
-    f = Fn / cE;
-    inv_Fn = 1.0 / Fn;
-  }
-  if (f > 1.0) f = 1.0;
-  const double f2 = f * f;
+  const bool cE_ok = cE > 1e-290 && cE < 1e290;
+  double r1 = fast_rcp(cE_ok ? cE : 1.0);
+  if (__any_sync(0xffffffffu, live && !cE_ok && E > 0.0)) r1 = cE_ok ? r1 : 1.0 / cE;   // rare: IEEE division
+  const double t0 = F0 * r1, t1 = F1 * r1, t2 = F2 * r1;
+  const double f2u = fma(t0, t0, fma(t1, t1, t2 * t2));                            // f^2 before the clamp
+  // isotropic when: Eddington closure, E <= 0, F = 0 (|F|^2 underflows exactly as the oracle's |F| does),
+  // or f^2 below the normal range (the anisotropic term is then < 1e-290 of the isotropic one)
+  const bool iso = closure == 1 || !(E > 0.0) || fma(F0, F0, fma(F1, F1, F2 * F2)) == 0.0 || !(f2u > 1e-290);
+  const double f2 = f2u > 1.0 ? 1.0 : f2u;
   const double chi = fma(4.0, f2, 3.0) * fast_rcp(fma(2.0, sqrt(fma(-3.0, f2, 4.0)), 5.0));
-  const double n0 = F0 * inv_Fn, n1 = F1 * inv_Fn, n2 = F2 * inv_Fn;
-  const double ndv = fma(n0, v0, fma(n1, v1, n2 * v2));
-  const double a = 0.5 * (1.0 - chi), b = 0.5 * fma(3.0, chi, -1.0) * ndv;
-  p0 = E * fma(a, v0, b * n0);
-  p1 = E * fma(a, v1, b * n1);
-  p2 = E * fma(a, v2, b * n2);
+  const double r2 = fast_rcp(iso || !(f2u < 1e290) ? 1.0 : f2u);
+  const double tv = fma(t0, v0, fma(t1, v1, t2 * v2));
+  const double a = iso ? 1.0 / 3.0 : 0.5 * (1.0 - chi);
+  const double b = 0.5 * fma(3.0, chi, -1.0) * tv * r2;
+  p0 = E * fma(a, v0, iso ? 0.0 : b * t0);       // (t may be inf/NaN on isotropic lanes: selected away)
+  p1 = E * fma(a, v1, iso ? 0.0 : b * t1);
+  p2 = E * fma(a, v2, iso ? 0.0 : b * t2);
 }
 
 // Lane phases of the flattened iteration.
@@ -377,9 +373,10 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
         if (!t0) { nFt0 = ft(0, 0); nFt1 = ft(1, 0); nFt2 = ft(2, 0); }
       }
 #pragma unroll 1
-      for (int i = 0; i < NQL; ++i) {
+      for (int i = 0; i < NQL; ++i) {      // executed by all lanes with per-lane predicates, like loop A
         const int g = i * L + sub - 1;
         const bool vg = fx && g >= 0 && g < Nq;
+        const int gi = g >= 0 && g < Nq ? g : 0;
         const double Et = nEt, Fk0 = nFk0, Fk1 = nFk1, Fk2 = nFk2;
         const double Ft0 = t0 ? nFk0 : nFt0, Ft1 = t0 ? nFk1 : nFt1, Ft2 = t0 ? nFk2 : nFt2;
         {
@@ -391,32 +388,33 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
             if (!t0) { nFt0 = ft(0, i + 1); nFt1 = ft(1, i + 1); nFt2 = ft(2, i + 1); }
           }
         }
+        const double R = sm(SL_R, i);
+        const double Enew = Et + R;                               // E_g^(t+1) = E_g^(t) + R_g
+        double p0, p1, p2;
+        closure_vP(P.closure, vg, Enew, Fk0, Fk1, Fk2, v0, v1, v2, c, p0, p1, p2);
+        const double w = P.onepa[gi] * (chis * P.k_mean[gi]);     // (1 + alpha) chi_E
+        const double chiF = sm(SL_CHIF, i), A = sm(SL_AG, i);
+        const double dn = fma(cdt, chiF, 1.0);                    // 1 + c_hat chi_F dt > 0 (guarded in A)
+        const bool dn_ok = dn > 1e-290 && dn < 1e290;
+        double inv_dn = fast_rcp(dn_ok ? dn : 1.0);
+        if (__any_sync(FULL, vg && !dn_ok)) inv_dn = dn_ok ? inv_dn : 1.0 / dn;
+        const double Fn0 = fma(cdt, fma(v0, A, w * p0), Ft0) * inv_dn;
+        const double Fn1 = fma(cdt, fma(v1, A, w * p1), Ft1) * inv_dn;
+        const double Fn2 = fma(cdt, fma(v2, A, w * p2), Ft2) * inv_dn;
+        const double e0 = Fn0 - Fk0, e1 = Fn1 - Fk1, e2 = Fn2 - Fk2;
+        const double d2 = fma(e0, e0, fma(e1, e1, e2 * e2));
+        const double f2 = fma(Fn0, Fn0, fma(Fn1, Fn1, Fn2 * Fn2));
+        // |dF| <= rel |F|, compared squared unless the squares leave the normal range
+        const bool sq_ok = f2 > 1e-280 && f2 < 1e280;
+        bool ok = d2 <= rel2 * f2;
+        if (__any_sync(FULL, vg && !sq_ok))
+          ok = sq_ok ? ok : norm3(e0, e1, e2) <= P.outer_rel_tol * norm3(Fn0, Fn1, Fn2);
         if (vg) {
           const long long o = (long long)g * stride + cell;
-          const double R = sm(SL_R, i);
           sumR += R;
           sumAbsR += fabs(R);
-          const double Enew = Et + R;                               // E_g^(t+1) = E_g^(t) + R_g
-          double p0, p1, p2;
-          closure_vP(P.closure, Enew, Fk0, Fk1, Fk2, v0, v1, v2, c, p0, p1, p2);
-          const double w = P.onepa[g] * (chis * P.k_mean[g]);       // (1 + alpha) chi_E
-          const double chiF = sm(SL_CHIF, i), A = sm(SL_AG, i);
-          const double dn = fma(cdt, chiF, 1.0);                    // 1 + c_hat chi_F dt > 0 (guarded in A)
-          const double inv_dn = (dn > 1e-290 && dn < 1e290) ? fast_rcp(dn) : 1.0 / dn;
-          const double Fn0 = fma(cdt, fma(v0, A, w * p0), Ft0) * inv_dn;
-          const double Fn1 = fma(cdt, fma(v1, A, w * p1), Ft1) * inv_dn;
-          const double Fn2 = fma(cdt, fma(v2, A, w * p2), Ft2) * inv_dn;
           dF0 += Fn0 - Ft0; dF1 += Fn1 - Ft1; dF2 += Fn2 - Ft2;
-          if (P.outer_stop == 1) {
-            const double e0 = Fn0 - Fk0, e1 = Fn1 - Fk1, e2 = Fn2 - Fk2;
-            const double d2 = fma(e0, e0, fma(e1, e1, e2 * e2));
-            const double f2 = fma(Fn0, Fn0, fma(Fn1, Fn1, Fn2 * Fn2));
-            // |dF| <= rel |F|, compared squared unless the squares leave the normal range
-            bool ok;
-            if (f2 > 1e-280 && f2 < 1e280) ok = d2 <= rel2 * f2;
-            else ok = norm3(e0, e1, e2) <= P.outer_rel_tol * norm3(Fn0, Fn1, Fn2);
-            if (!ok) rel_bad = 1;
-          }
+          if (P.outer_stop == 1 && !ok) rel_bad = 1;
           if (t0) { ft(0, i) = Ft0; ft(1, i) = Ft1; ft(2, i) = Ft2; }
           S.Frad[0][o] = Fn0; S.Frad[1][o] = Fn1; S.Frad[2][o] = Fn2;   // lagged flux of the next trip, in place
           sm(SL_DA, i) = Fn0; sm(SL_DB, i) = Fn1; sm(SL_AG, i) = Fn2;   // kept on chip for loop C
