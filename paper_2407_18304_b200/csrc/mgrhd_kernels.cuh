@@ -226,16 +226,23 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
       const int src = sub == 0 ? lane + (L - 1) : lane - 1;   // lane that owns the lower edge
       const bool last = sub == L - 1;
       const bool evf = ev && first, evp = ev && pend;
-      // register prefetch of the next step's global operands (group g = e - 1, e = i*L + sub)
+      // register prefetch of the next step's global operands (group g = e - 1, e = i*L + sub).
+      // Byte offsets of (group, cell) advance by a warp-uniform stride per step, so each stream
+      // costs one 64-bit add and one load.
+      const char* const pE = reinterpret_cast<const char*>(S.Erad);
+      const char* const pF0 = reinterpret_cast<const char*>(S.Frad[0]);
+      const char* const pF1 = reinterpret_cast<const char*>(S.Frad[1]);
+      const char* const pF2 = reinterpret_cast<const char*>(S.Frad[2]);
+      const long long dstep = (long long)L * stride * 8;
+      long long oc = ((long long)(sub - 1) * stride + cell) * 8;        // (g, cell) of the step being loaded
+      long long of = ((long long)(sub - 1) * stride + fin_cell) * 8;    // (g, fin_cell)
+      long long of_cur = of;
       double nEt = 0.0, nF0 = 0.0, nF1 = 0.0, nF2 = 0.0, nEo = 0.0;
-      {
-        const int g0 = sub - 1;
-        if (g0 >= 0 && g0 < Nq) {
-          const long long o = (long long)g0 * stride;
-          if (ev) nEt = S.Erad[o + cell];
-          if (evf) { nF0 = S.Frad[0][o + cell]; nF1 = S.Frad[1][o + cell]; nF2 = S.Frad[2][o + cell]; }
-          if (fin) nEo = S.Erad[o + fin_cell];
-        }
+      auto ldd = [](const char* p, long long o) { return *reinterpret_cast<const double*>(p + o); };
+      if (sub >= 1 && sub - 1 < Nq) {
+        if (ev) nEt = ldd(pE, oc);
+        if (evf) { nF0 = ldd(pF0, oc); nF1 = ldd(pF1, oc); nF2 = ldd(pF2, oc); }
+        if (fin) nEo = ldd(pE, of);
       }
       // The body below is executed by ALL lanes of the warp with per-lane predicates (a lane
       // without a cell or without a group in this step computes on harmless values and stores
@@ -248,18 +255,17 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
         const bool evg = ev && vg;
         const int gi = vg ? g : 0;                   // safe table index
         const double Et = nEt, F0 = nF0, F1 = nF1, F2 = nF2, Eo = nEo;
-        {
-          const int g1 = g + L;
-          if (g1 >= 0 && g1 < Nq) {
-            const long long o1 = (long long)g1 * stride;
-            if (ev) nEt = S.Erad[o1 + cell];
-            if (evf) { nF0 = S.Frad[0][o1 + cell]; nF1 = S.Frad[1][o1 + cell]; nF2 = S.Frad[2][o1 + cell]; }
-            if (fin) nEo = S.Erad[o1 + fin_cell];
-          }
+        of_cur = of;
+        oc += dstep;
+        of += dstep;
+        if (g + L >= 0 && g + L < Nq) {
+          if (ev) nEt = ldd(pE, oc);
+          if (evf) { nF0 = ldd(pF0, oc); nF1 = ldd(pF1, oc); nF2 = ldd(pF2, oc); }
+          if (fin) nEo = ldd(pE, of);
         }
         const double Rold = sm(SL_R, i);
         // a10 of the cell this lane finished in the previous trip: E_g^(t+1) = E_g^(t) + R_g
-        if (fin && vg) S.Erad[(long long)g * stride + fin_cell] = Eo + Rold;
+        if (fin && vg) *reinterpret_cast<double*>(const_cast<char*>(pE) + of_cur) = Eo + Rold;
         // a1: edge functions at this lane's edge; the lower edge of group g comes from the left
         double hi_yz, hi_xi;
         bool hi_small;
@@ -365,11 +371,17 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
       const double v0 = momk0 * inv_rho, v1 = momk1 * inv_rho, v2 = momk2 * inv_rho;
       double sumR = 0.0, sumAbsR = 0.0, dF0 = 0.0, dF1 = 0.0, dF2 = 0.0;
       int rel_bad = 0;
+      char* const pE = reinterpret_cast<char*>(S.Erad);
+      char* const pF0 = reinterpret_cast<char*>(S.Frad[0]);
+      char* const pF1 = reinterpret_cast<char*>(S.Frad[1]);
+      char* const pF2 = reinterpret_cast<char*>(S.Frad[2]);
+      const long long dstep = (long long)L * stride * 8;
+      long long oc = ((long long)(sub - 1) * stride + cell) * 8, oc_cur = oc;
+      auto ldd = [](const char* p, long long o) { return *reinterpret_cast<const double*>(p + o); };
       double nEt = 0.0, nFt0 = 0.0, nFt1 = 0.0, nFt2 = 0.0, nFk0 = 0.0, nFk1 = 0.0, nFk2 = 0.0;
       if (fx && sub >= 1 && sub - 1 < Nq) {
-        const long long o = (long long)(sub - 1) * stride + cell;
-        nEt = S.Erad[o];
-        nFk0 = S.Frad[0][o]; nFk1 = S.Frad[1][o]; nFk2 = S.Frad[2][o];
+        nEt = ldd(pE, oc);
+        nFk0 = ldd(pF0, oc); nFk1 = ldd(pF1, oc); nFk2 = ldd(pF2, oc);
         if (!t0) { nFt0 = ft(0, 0); nFt1 = ft(1, 0); nFt2 = ft(2, 0); }
       }
 #pragma unroll 1
@@ -379,14 +391,12 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
         const int gi = g >= 0 && g < Nq ? g : 0;
         const double Et = nEt, Fk0 = nFk0, Fk1 = nFk1, Fk2 = nFk2;
         const double Ft0 = t0 ? nFk0 : nFt0, Ft1 = t0 ? nFk1 : nFt1, Ft2 = t0 ? nFk2 : nFt2;
-        {
-          const int g1 = g + L;
-          if (fx && g1 >= 0 && g1 < Nq) {
-            const long long o1 = (long long)g1 * stride + cell;
-            nEt = S.Erad[o1];
-            nFk0 = S.Frad[0][o1]; nFk1 = S.Frad[1][o1]; nFk2 = S.Frad[2][o1];
-            if (!t0) { nFt0 = ft(0, i + 1); nFt1 = ft(1, i + 1); nFt2 = ft(2, i + 1); }
-          }
+        oc_cur = oc;
+        oc += dstep;
+        if (fx && g + L >= 0 && g + L < Nq) {
+          nEt = ldd(pE, oc);
+          nFk0 = ldd(pF0, oc); nFk1 = ldd(pF1, oc); nFk2 = ldd(pF2, oc);
+          if (!t0) { nFt0 = ft(0, i + 1); nFt1 = ft(1, i + 1); nFt2 = ft(2, i + 1); }
         }
         const double R = sm(SL_R, i);
         const double Enew = Et + R;                               // E_g^(t+1) = E_g^(t) + R_g
@@ -410,13 +420,15 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
         if (__any_sync(FULL, vg && !sq_ok))
           ok = sq_ok ? ok : norm3(e0, e1, e2) <= P.outer_rel_tol * norm3(Fn0, Fn1, Fn2);
         if (vg) {
-          const long long o = (long long)g * stride + cell;
           sumR += R;
           sumAbsR += fabs(R);
           dF0 += Fn0 - Ft0; dF1 += Fn1 - Ft1; dF2 += Fn2 - Ft2;
           if (P.outer_stop == 1 && !ok) rel_bad = 1;
           if (t0) { ft(0, i) = Ft0; ft(1, i) = Ft1; ft(2, i) = Ft2; }
-          S.Frad[0][o] = Fn0; S.Frad[1][o] = Fn1; S.Frad[2][o] = Fn2;   // lagged flux of the next trip, in place
+          // lagged flux of the next trip, in place
+          *reinterpret_cast<double*>(pF0 + oc_cur) = Fn0;
+          *reinterpret_cast<double*>(pF1 + oc_cur) = Fn1;
+          *reinterpret_cast<double*>(pF2 + oc_cur) = Fn2;
           sm(SL_DA, i) = Fn0; sm(SL_DB, i) = Fn1; sm(SL_AG, i) = Fn2;   // kept on chip for loop C
         }
       }

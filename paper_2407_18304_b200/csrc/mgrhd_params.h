@@ -85,7 +85,7 @@ constexpr int kLargeTerms = 7;    // terms of the e^{-nx} series, x >= kXL
 constexpr double kXS = 1.25;
 constexpr double kXL = 5.5;
 // Coefficients are stored in PAIRS (one 16-byte constant load feeds both Horner chains).
-struct Pair { double a, b; };
+struct alignas(16) Pair { double a, b; };
 struct alignas(16) PlanckTables {
   // t/(e^t-1) = 1 - t/2 + sum_{n>=1} b_{2n} t^(2n),  b_{2n} = B_{2n}/(2n)!
   //   sp[n-1] = { b_{2n}/(2n+3), b_{2n} } :  Y(x)  = C x^3 (1/3 - x/8 + sum sp[n-1].a x^(2n)),

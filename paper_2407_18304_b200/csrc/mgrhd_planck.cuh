@@ -140,6 +140,9 @@ __device__ __forceinline__ EdgeFn planck_edge(double x, TableBase tb) {
 // datapath, two coefficients per load, with no reconvergence bookkeeping.  `which` must be
 // warp-uniform and change with the caller's loop counter (see TableBase above).
 // x = NaN marks a lane without an edge: it matches no branch and gets (0, 0, large).
+// One 16-byte load of a coefficient pair.
+__device__ __forceinline__ double2 ld_pair(const Pair& p) { return *reinterpret_cast<const double2*>(&p); }
+
 __device__ __forceinline__ void planck_edge_w(double x, int which, double& yz, double& xi, bool& small,
                                               int& flops) {
   const PlanckTables& tb = mgrhd_c_planck[which & 1];
@@ -150,11 +153,13 @@ __device__ __forceinline__ void planck_edge_w(double x, int which, double& yz, d
   yz = 0.0; xi = 0.0; small = inS; flops = 0;
   if (__any_sync(FULL, inS)) {
     const double x2 = x * x;
-    double sy = tb.sp[kSmallTerms - 1].a, sx = tb.sp[kSmallTerms - 1].b;
+    double2 cf = ld_pair(tb.sp[kSmallTerms - 1]);
+    double sy = cf.x, sx = cf.y;
 #pragma unroll
     for (int n = kSmallTerms - 2; n >= 0; --n) {
-      sy = fma(sy, x2, tb.sp[n].a);
-      sx = fma(sx, x2, tb.sp[n].b);
+      cf = ld_pair(tb.sp[n]);
+      sy = fma(sy, x2, cf.x);
+      sx = fma(sx, x2, cf.y);
     }
     const double cx3 = kC15Pi4 * (x2 * x);
     // Y = C x^3 (1/3 - x/8 + x^2 sy),  Xi = C x^3 (1 - x/2 + x^2 sx)
@@ -164,11 +169,13 @@ __device__ __forceinline__ void planck_edge_w(double x, int which, double& yz, d
   }
   if (__any_sync(FULL, inM)) {
     const double t = fma(x, tb.mid_s, tb.mid_o);
-    double sz = tb.mp[kMidTerms - 1].a, sx = tb.mp[kMidTerms - 1].b;
+    double2 cf = ld_pair(tb.mp[kMidTerms - 1]);
+    double sz = cf.x, sx = cf.y;
 #pragma unroll
     for (int n = kMidTerms - 2; n >= 0; --n) {
-      sz = fma(sz, t, tb.mp[n].a);
-      sx = fma(sx, t, tb.mp[n].b);
+      cf = ld_pair(tb.mp[n]);
+      sz = fma(sz, t, cf.x);
+      sx = fma(sx, t, cf.y);
     }
     if (inM) { yz = sz; xi = sx; flops = kFlopEdgeMid; }
   }
@@ -178,7 +185,8 @@ __device__ __forceinline__ void planck_edge_w(double x, int which, double& yz, d
     double sum = 0.0;
 #pragma unroll
     for (int n = kLargeTerms - 1; n >= 0; --n) {
-      const double pn = fma(fma(fma(tb.l32[n].a, xx, tb.l32[n].b), xx, tb.l10[n].a), xx, tb.l10[n].b);
+      const double2 c32 = ld_pair(tb.l32[n]), c10 = ld_pair(tb.l10[n]);
+      const double pn = fma(fma(fma(c32.x, xx, c32.y), xx, c10.x), xx, c10.y);
       sum = fma(sum, u, pn);
     }
     const double x2 = xx * xx;
