@@ -48,19 +48,21 @@ __device__ __forceinline__ double norm3(double a, double b, double c) {
 // v^j P^{ji} for one group (closure reading S7 of DESIGN.md): Levermore/M1
 // or Eddington P = E/3 I.  Branch-free for a converged warp: with t = F/(cE),
 // f^2 = |t|^2 and n (n.v) = t (t.v)/f^2, so neither |F| nor a unit vector is formed.
-// `live` marks lanes whose result is used (the others may hold anything).
-__device__ __forceinline__ void closure_vP(int closure, bool live, double E, double F0, double F1, double F2,
+__device__ __forceinline__ void closure_vP(int closure, double E, double F0, double F1, double F2,
                                            double v0, double v1, double v2, double c,
                                            double& p0, double& p1, double& p2) {
-  const double cE = c * E;
-  const bool cE_ok = cE > 1e-290 && cE < 1e290;
-  double r1 = fast_rcp(cE_ok ? cE : 1.0);
-  if (__any_sync(0xffffffffu, live && !cE_ok && E > 0.0)) r1 = cE_ok ? r1 : 1.0 / cE;   // rare: IEEE division
+  // tail groups hold E ~ 1e-300 and below: scale F and cE by an exact power of two into the normal range
+  const double cE0 = c * E;
+  const double sc = cE0 < 1e-200 ? 0x1p+400 : (cE0 > 1e200 ? 0x1p-400 : 1.0);
+  const double cE = cE0 * sc;
+  const bool Fzero = fma(F0, F0, fma(F1, F1, F2 * F2)) == 0.0;   // |F| = 0, with the oracle's underflow
+  F0 *= sc; F1 *= sc; F2 *= sc;
+  const double r1 = fast_rcp(cE > 0.0 ? cE : 1.0);
   const double t0 = F0 * r1, t1 = F1 * r1, t2 = F2 * r1;
   const double f2u = fma(t0, t0, fma(t1, t1, t2 * t2));                            // f^2 before the clamp
   // isotropic when: Eddington closure, E <= 0, F = 0 (|F|^2 underflows exactly as the oracle's |F| does),
   // or f^2 below the normal range (the anisotropic term is then < 1e-290 of the isotropic one)
-  const bool iso = closure == 1 || !(E > 0.0) || fma(F0, F0, fma(F1, F1, F2 * F2)) == 0.0 || !(f2u > 1e-290);
+  const bool iso = closure == 1 || !(E > 0.0) || Fzero || !(f2u > 1e-290);
   const double f2 = f2u > 1.0 ? 1.0 : f2u;
   const double chi = fma(4.0, f2, 3.0) * fast_rcp(fma(2.0, sqrt(fma(-3.0, f2, 4.0)), 5.0));
   const double r2 = fast_rcp(iso || !(f2u < 1e290) ? 1.0 : f2u);
@@ -217,7 +219,6 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
       const double beta = P.h_over_k * invT;
       const double itau_c = inv_chis / cdt;          // 1/(c_hat dt chi_E,g) = itau_c * inv_k_mean[g]
       const double dBscale = invT * inv_Cv;          // J_g0 = (4 Bt - Db) / (T C_v), Eq. 46
-      const double guard_thr = 1e-280 * aT4;
       const double v0 = momk0 * inv_rho, v1 = momk1 * inv_rho, v2 = momk2 * inv_rho;
       double sumR = 0.0, sumAbsFR = 0.0, SFRq = 0.0, SJq = 0.0, sumEt = 0.0;
       int eflops = 0;
@@ -289,26 +290,26 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
         if (first) { R = 0.0; vF = fma(v0, F0, fma(v1, F1, v2 * F2)); }
         if (evg) { sm(SL_R, i) = R; sm(SL_VF, i) = vF; }
         if (evf && vg) sumEt += Et;
-        // a2: group Planck integral and Doppler boundary terms (Eq. 11, 18, 22)
+        // a2: group Planck integral and Doppler boundary terms (Eq. 11, 18, 22), per unit a_R T^4.
+        // chi_F is formed from the UNSCALED differences dY, dXi (a_R T^4 cancels in Eq. 27), so its
+        // denominator is in [1e-280, 4/3] whenever the Wien guard does not fire and the fast
+        // reciprocal is always valid: no slow path, no branch.
         const double dY = hi_small ? hi_yz - lo_yz : (lo_small ? (1.0 - lo_yz) - hi_yz : lo_yz - hi_yz);
-        const double Bt = aT4 * dY;
-        const double Db = aT4 * (hi_xi - lo_xi);
-        const double D = aT4 * chis * fma(P.k_hi[gi], hi_xi, -P.k_lo[gi] * lo_xi);
+        const double dX = hi_xi - lo_xi;
+        const double Dp3 = chis * fma(P.k_hi[gi], hi_xi, -P.k_lo[gi] * lo_xi) * (1.0 / 3.0);
         const double chiE = chis * P.k_mean[gi];                 // = chi_B (alpha_Q = -1 for both)
-        const double fourBmDb = fma(4.0, Bt, -Db);               // 3 x denominator of Eq. 27 = T dBt/dT
+        const double fbd = fma(4.0, dY, -dX);                    // 3 x denominator of Eq. 27 = T dBt/dT / (a_R T^4)
         // a3: flux-mean opacity, Eq. 27, with the Wien-limit guard (S8)
-        const double den = fourBmDb * (1.0 / 3.0);
-        const double Dthird = D * (1.0 / 3.0);
-        const double num = fma(chis * Bt, P.k_num[gi], -Dthird); // (chi_B + chi_E/3 + alpha chi_E/3) Bt - D/3
-        const bool guard = !(den >= guard_thr) || isinf(den);
-        const bool den_normal = den > 1e-290 && den < 1e290;
-        double chiF = num * fast_rcp(den_normal ? den : 1.0);
-        if (__any_sync(FULL, evg && !guard && !den_normal)) chiF = den_normal ? chiF : num / den;   // rare: IEEE division
+        const double den = fbd * (1.0 / 3.0);
+        const double num = fma(chis * dY, P.k_num[gi], -Dp3);    // (chi_B + chi_E/3 + alpha chi_E/3) dY - D/3
+        const bool guard = !(den >= 1e-280) || isinf(aT4 * den);
+        double chiF = num * fast_rcp(guard ? 1.0 : den);
         if (guard) chiF = chis * P.k_lo[gi];
         const bool denbad = !(fma(cdt, chiF, 1.0) > 0.0);
         if (denbad) chiF = chiE;
         if (evg && evals == 0) { cnt_guard += guard ? 1u : 0u; cnt_den += denbad ? 1u : 0u; }
         // a4: residuals (Eq. 41; Eq. 42 solved for E_g)
+        const double Bt = aT4 * dY;
         const double inv_chiE = inv_chis * P.inv_k_mean[gi];
         const double itau = itau_c * P.inv_k_mean[gi];
         const double W = P.onepa[gi] * chiF * vF * inv_c;
@@ -316,7 +317,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
         const double FR = Eg - Et - R;
         // a5: Jacobian (Eq. 44-47) folded into the arrowhead elimination (Eq. 48): 1/J_gg = -q
         const double q = fast_rcp(1.0 + itau);
-        const double da = FR * q, db = fourBmDb * dBscale * q;
+        const double da = FR * q, db = aT4 * fbd * dBscale * q;
         if (evg) {
           sumR += R;
           sumAbsFR += fabs(FR);
@@ -324,7 +325,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
           SJq += db;
           sm(SL_DA, i) = da;
           sm(SL_DB, i) = db;
-          sm(SL_AG, i) = fma(chiE, Bt, -Dthird);                 // chi_B Bt - D/3 (Eq. 51 source)
+          sm(SL_AG, i) = aT4 * fma(chiE, dY, -Dp3);              // chi_B Bt - D/3 (Eq. 51 source)
           sm(SL_CHIF, i) = chiF;
         }
       }
@@ -401,7 +402,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
         const double R = sm(SL_R, i);
         const double Enew = Et + R;                               // E_g^(t+1) = E_g^(t) + R_g
         double p0, p1, p2;
-        closure_vP(P.closure, vg, Enew, Fk0, Fk1, Fk2, v0, v1, v2, c, p0, p1, p2);
+        closure_vP(P.closure, Enew, Fk0, Fk1, Fk2, v0, v1, v2, c, p0, p1, p2);
         const double w = P.onepa[gi] * (chis * P.k_mean[gi]);     // (1 + alpha) chi_E
         const double chiF = sm(SL_CHIF, i), A = sm(SL_AG, i);
         const double dn = fma(cdt, chiF, 1.0);                    // 1 + c_hat chi_F dt > 0 (guarded in A)

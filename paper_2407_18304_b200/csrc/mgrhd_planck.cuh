@@ -201,6 +201,68 @@ __device__ __forceinline__ void planck_edge_w(double x, int which, double& yz, d
   }
 }
 
+// Two edges at once (the same lane's edges of two consecutive steps): a branch needed by either
+// edge of any lane is executed for BOTH edges by all lanes, so the four Horner chains interleave
+// (DFMA latency is 8 cycles; two chains per warp leave the FP64 pipe half idle at 8 warps/SM) and
+// each coefficient load feeds four DFMAs.
+struct EdgeVal { double yz, xi; bool small; int flops; };
+
+__device__ __forceinline__ void planck_edge_w2(double xa, double xb, int which, EdgeVal& A, EdgeVal& B) {
+  const PlanckTables& tb = mgrhd_c_planck[which & 1];
+  const unsigned FULL = 0xffffffffu;
+  const bool aS = xa < kXS, aM = xa >= kXS && xa < kXL, aL = xa >= kXL;
+  const bool bS = xb < kXS, bM = xb >= kXS && xb < kXL, bL = xb >= kXL;
+  A.yz = 0.0; A.xi = 0.0; A.small = aS; A.flops = 0;
+  B.yz = 0.0; B.xi = 0.0; B.small = bS; B.flops = 0;
+  if (__any_sync(FULL, aS || bS)) {
+    const double a2 = xa * xa, b2 = xb * xb;
+    double2 cf = ld_pair(tb.sp[kSmallTerms - 1]);
+    double ya = cf.x, za = cf.y, yb = cf.x, zb = cf.y;
+#pragma unroll
+    for (int n = kSmallTerms - 2; n >= 0; --n) {
+      cf = ld_pair(tb.sp[n]);
+      ya = fma(ya, a2, cf.x); za = fma(za, a2, cf.y);
+      yb = fma(yb, b2, cf.x); zb = fma(zb, b2, cf.y);
+    }
+    const double ca3 = kC15Pi4 * (a2 * xa), cb3 = kC15Pi4 * (b2 * xb);
+    // Y = C x^3 (1/3 - x/8 + x^2 sy),  Xi = C x^3 (1 - x/2 + x^2 sx)
+    ya = ca3 * fma(a2, ya, fma(-0.125, xa, 1.0 / 3.0)); za = ca3 * fma(a2, za, fma(-0.5, xa, 1.0));
+    yb = cb3 * fma(b2, yb, fma(-0.125, xb, 1.0 / 3.0)); zb = cb3 * fma(b2, zb, fma(-0.5, xb, 1.0));
+    if (aS) { A.yz = ya; A.xi = za; A.flops = kFlopEdgeSmall; }
+    if (bS) { B.yz = yb; B.xi = zb; B.flops = kFlopEdgeSmall; }
+  }
+  if (__any_sync(FULL, aM || bM)) {
+    const double ta = fma(xa, tb.mid_s, tb.mid_o), tbb = fma(xb, tb.mid_s, tb.mid_o);
+    double2 cf = ld_pair(tb.mp[kMidTerms - 1]);
+    double za = cf.x, wa = cf.y, zb = cf.x, wb = cf.y;
+#pragma unroll
+    for (int n = kMidTerms - 2; n >= 0; --n) {
+      cf = ld_pair(tb.mp[n]);
+      za = fma(za, ta, cf.x); wa = fma(wa, ta, cf.y);
+      zb = fma(zb, tbb, cf.x); wb = fma(wb, tbb, cf.y);
+    }
+    if (aM) { A.yz = za; A.xi = wa; A.flops = kFlopEdgeMid; }
+    if (bM) { B.yz = zb; B.xi = wb; B.flops = kFlopEdgeMid; }
+  }
+  if (__any_sync(FULL, aL || bL)) {
+    const double ua = exp(-xa), ub = exp(-xb);            // 0 on underflow and for x = +inf
+    const double pa = aL && ua > 0.0 ? xa : 1.0;          // keeps inf * 0 out of the polynomials
+    const double pb = bL && ub > 0.0 ? xb : 1.0;
+    double sa = 0.0, sb = 0.0;
+#pragma unroll
+    for (int n = kLargeTerms - 1; n >= 0; --n) {
+      const double2 c32 = ld_pair(tb.l32[n]), c10 = ld_pair(tb.l10[n]);
+      sa = fma(sa, ua, fma(fma(fma(c32.x, pa, c32.y), pa, c10.x), pa, c10.y));
+      sb = fma(sb, ub, fma(fma(fma(c32.x, pb, c32.y), pb, c10.x), pb, c10.y));
+    }
+    const double a2 = pa * pa, b2 = pb * pb;
+    const double wa = kC15Pi4 * (a2 * a2) * (ua * fast_rcp(1.0 - ua));
+    const double wb = kC15Pi4 * (b2 * b2) * (ub * fast_rcp(1.0 - ub));
+    if (aL) { const bool l = ua > 0.0; A.yz = l ? sa * ua : 0.0; A.xi = l ? wa : 0.0; A.flops = l ? kFlopEdgeLarge : kFlopEdgeZero; }
+    if (bL) { const bool l = ub > 0.0; B.yz = l ? sb * ub : 0.0; B.xi = l ? wb : 0.0; B.flops = l ? kFlopEdgeLarge : kFlopEdgeZero; }
+  }
+}
+
 // Y(hi) - Y(lo) for two edges of one group (lo below hi).
 __device__ __forceinline__ double planck_dY(const EdgeFn& lo, const EdgeFn& hi) {
   if (hi.small) return hi.yz - lo.yz;          // both small
