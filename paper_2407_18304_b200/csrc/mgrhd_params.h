@@ -28,21 +28,23 @@ enum StatSlot {
   kStatCount = kStatOuterHist + MGRHD_HIST
 };
 
-// Algorithmic FP64 flop counts of each piece of the update as written in mgrhd_kernels.cuh
-// (FMA = 2; add, mul, div, sqrt = 1; exp = kFlopExp; comparisons, fabs, selects = 0).
-// Derived line by line in DESIGN.md "Algorithmic flops"; used only by the counting kernels.
-constexpr int kFlopExp = 30;          // range reduction + degree-11 polynomial + scaling
-constexpr int kFlopEdgeSmall = 59;    // x < kXS: two 12-term Horner chains in x^2 + assembly
-constexpr int kFlopEdgeMid = 95;      // kXS <= x < kXL: two degree-23 Horner chains
-constexpr int kFlopEdgeLarge = 94;    // x >= kXL: exp, 7 terms (3+1 FMA each), Xi with one reciprocal
-constexpr int kFlopEdgeZero = 32;     // e^{-x} underflowed
-constexpr int kFlopGroupEval = 62;    // a2-a5 for one group at one trial T
-constexpr int kFlopCellEval = 13;     // T, a_R T^4, beta, F_G, Eq. 49
-constexpr int kFlopStepCell = 9;      // dx0, T>0 check, E_gas update
-constexpr int kFlopStepGroup = 4;     // R_g += lam (da + db dx0)
-constexpr int kFlopOuterCell = 45;    // v, E_kin, commit, Eq. 52, outer test
-constexpr int kFlopOuterGroup = 106;  // closure, Eq. 51, relative-change test, next v.F_g, dW
-constexpr int kFlopCell = 6;          // load-time derivations
+// Algorithmic FP64 flop counts of each piece of the update as written in mgrhd_kernels.cuh and
+// mgrhd_planck.cuh (FMA = 2; add, mul, reciprocal/divide, sqrt = 1; exp = 30; comparisons, fabs,
+// selects, shuffles = 0).  Derived line by line in DESIGN.md section 8; used only by the
+// counting instantiations of the kernel (mgrhd_set_flop_counting), never in a timed run.
+// A lane is charged for the ONE edge-function branch its x falls in, not for the branches it
+// executes on behalf of other lanes of its warp.
+constexpr int kFlopEdgeSmall = 59;    // x < kXS: x, x^2, two 12-term Horner chains in x^2, assembly
+constexpr int kFlopEdgeMid = 95;      // kXS <= x < kXL: x, t, two degree-23 Horner chains
+constexpr int kFlopEdgeLarge = 96;    // x >= kXL: x, exp, 7 terms of (3+1) FMA, Xi with one reciprocal
+constexpr int kFlopEdgeZero = 32;     // x, exp that underflowed
+constexpr int kFlopGroupEval = 47;    // a2-a5 for one group at one trial T
+constexpr int kFlopCellEval = 24;     // T, a_R T^4, beta, scales, v, F_G, Eq. 49, sums over the cell's lanes
+constexpr int kFlopStepCell = 10;     // dx0, T > 0 check, E_gas update
+constexpr int kFlopStepGroup = 4;     // R_g += lam da_g + (lam dx0) db_g
+constexpr int kFlopOuterCell = 50;    // v, Eq. 52, commit, E_kin, outer tests, sums over the cell's lanes
+constexpr int kFlopOuterGroup = 109;  // closure (53), Eq. 51 (23), relative-change test (14), sums (9), next v.F_g and dW (10)
+constexpr int kFlopCell = 16;         // load-time derivations
 constexpr int kFlopCellGroup = 7;     // sum E_g, first v.F_g, E_g commit
 
 struct Params {
