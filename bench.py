@@ -275,7 +275,8 @@ def run_ours(args) -> None:
     hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
     roofline = {
         "bound": "alu", "achieved": achieved_tflops, "peak": peak_tflops, "unit": "TFLOP/s",
-        "frac": achieved_tflops / peak_tflops, "traffic": NCU_TRAFFIC_BYTES.get(wl.index),
+        "frac": achieved_tflops / peak_tflops,
+        "traffic": NCU_TRAFFIC_BYTES.get(wl.index) if n == W.workload(wl.index).ncells else None,
         "peak_source": "FP64 FMA rate measured in this run by mgrhd_measure_dfma_peak (x2 flop/FMA)",
         "algorithmic_flops_per_launch": flops_per_launch,
         "algorithmic_flops_per_cell_group": flops_per_launch / (n * Nq),
@@ -322,8 +323,10 @@ def run_ours(args) -> None:
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the update kernel, from the
-# `ncu --set full` capture summarised under profiles/ (None until a capture of that workload exists).
-NCU_TRAFFIC_BYTES: dict = {}
+# `ncu --set full` capture summarised in profiles/r1_v7_ncu_full.md: 2.667 + 6.066 GB at
+# 2 097 152 cells of config 4, scaled x8 to its 16 777 216 cells (persistent grid-stride kernel,
+# traffic linear in cells).  None for workloads without a capture.
+NCU_TRAFFIC_BYTES: dict = {4: 8.0 * (2.666830e9 + 6.066333e9)}
 
 
 def run_e2e(args, wl, ctx, pristine, dt, world, dist):
