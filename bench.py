@@ -36,6 +36,9 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--cpu-sample-cells", type=int, default=None)
+    ap.add_argument("--sustained", type=int, default=0, metavar="CALLS",
+                    help="BASELINE.json config 5 as stated: CALLS successive updates of the same buffers, dt varied "
+                         "per call, device-timed per call, conservation residuals checked after every call")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -396,10 +399,75 @@ def run_cpu_baseline(args, wl, pristine, work, dt):
     return cpu, parity
 
 
+def run_sustained(args) -> None:
+    """Config 5 as BASELINE.json states it: successive updates on the same buffers (no restore), dt_i = dt0 *
+    10^U[-.5,.5], one CUDA-event pair per call, conservation residuals reduced on the device after every call."""
+    import torch
+
+    from paper_2407_18304_b200 import binding, build, workloads as W
+
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    build.build()
+    wl = W.workload(5, ncells=args.cells)
+    n, Nq, calls = wl.ncells, wl.Nq, args.sustained
+    st = wl.make_state(device="cuda")
+    ctx = binding.Context.from_workload(wl)
+    stream = torch.cuda.current_stream()
+    E0 = torch.empty(n, dtype=torch.float64, device="cuda")
+    P0 = torch.empty(3, n, dtype=torch.float64, device="cuda")
+    E1, P1 = torch.empty_like(E0), torch.empty_like(P0)
+    resE = torch.zeros(calls, dtype=torch.float64, device="cuda")
+    resP = torch.zeros(calls, dtype=torch.float64, device="cuda")
+    sampler = ClockSampler(0)
+    sampler.start()
+    evs, launches0 = [], ctx.launch_count()
+    for i in range(calls):
+        dt = wl.dt_of_call(i)
+        ctx.conserved_totals(st, wl.c, wl.c_hat, E0, P0)
+        Es = st["Egas"].abs() + (wl.c / wl.c_hat) * st["Erad"].abs().sum(0)
+        Ps = st["mom"].pow(2).sum(0).sqrt() + st["Frad"].pow(2).sum(0).sqrt().sum(0) / (wl.c * wl.c_hat)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        ctx.source_update(st, dt, wl.c, wl.c_hat)
+        e1.record(stream)
+        evs.append((e0, e1))
+        ctx.conserved_totals(st, wl.c, wl.c_hat, E1, P1)
+        resE[i] = ((E1 - E0).abs() / Es).max()
+        dP = (P1 - P0).pow(2).sum(0).sqrt()
+        resP[i] = torch.where(Ps > 0, dP / Ps, dP).max()
+        del Es, Ps, dP
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    ms = [a.elapsed_time(b) for a, b in evs]
+    stats = ctx.get_stats()
+    total_s = sum(ms) * 1e-3
+    line = {
+        "metric": METRIC, "value": n * Nq * calls / total_s, "unit": UNIT, "n_gpus": 1, "steps": calls, "warmup": 0,
+        "ms_per_step": 1e3 * total_s / calls, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_label(wl) + " (sustained: successive calls, no restore)", "cells_per_gpu": n,
+                   "Nq": Nq, "c": wl.c, "c_hat": wl.c_hat, "l2": "state larger than L2"},
+        "clocks": clocks, "gpu_launches": (ctx.launch_count() - launches0 - 2 * calls),
+        "call_ms": {"first": ms[0], "min": min(ms), "max": max(ms), "last": ms[-1]},
+        "iterations": {"newton_evals_per_cell_call": stats["newton_evals_total"] / (n * calls),
+                       "outer_trips_per_cell_call": stats["outer_trips_total"] / (n * calls),
+                       "n_newton_unconverged": stats["n_newton_unconverged"],
+                       "n_outer_unconverged": stats["n_outer_unconverged"]},
+        "conservation": {"energy_residual_max_over_calls": float(resE.max()),
+                         "momentum_residual_max_over_calls": float(resP.max()),
+                         "all_finite": all(bool(torch.isfinite(st[k]).all()) for k in ("mom", "Egas", "Erad", "Frad"))},
+    }
+    ctx.free()
+    print(json.dumps(line))
+
+
 def main():
     args = parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.sustained > 0:
+        run_sustained(args)
     else:
         run_ours(args)
 
