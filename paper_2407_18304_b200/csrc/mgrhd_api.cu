@@ -142,7 +142,7 @@ struct mgrhd_ctx {
   cudaStream_t last_stream;
   long long launches;
   int count_flops;
-  int variant, cfg_l;
+  int cfg_l;
   int cfg_nq, cfg_threads, cfg_bps;   // kernel instantiation, CTA size, resident CTAs per SM
   double* scratch;                    // lagged-flux scratch of the device path
   double* slab_scratch[kSlabs];       // ... and of each host-path slab stream
@@ -176,32 +176,22 @@ struct Inst {
   }
 };
 
-// WHAT(L, NQL, THREADS); V = MGRHD_VARIANT (tuning experiments only; 0 = default)
-#define MGRHD_DISPATCH(Nq, V, WHAT)                            \
+// WHAT(L, NQL, THREADS): lanes per cell, steps per lane (L*NQL >= Nq+1), CTA size -- measured best
+// on B200 for each bracket of Nq.
+#define MGRHD_DISPATCH(Nq, WHAT)                               \
   do {                                                         \
     if ((Nq) <= 4) { WHAT(1, 5, 256); }                        \
     else if ((Nq) <= 8) { WHAT(1, 9, 256); }                   \
-    else if ((Nq) <= 16) { WHAT(1, 17, 256); }                 \
-    else if ((Nq) <= 32) {                                     \
-      if ((V) == 1) { WHAT(2, 17, 256); }                      \
-      else if ((V) == 2) { WHAT(4, 9, 512); }                  \
-      else if ((V) == 3) { WHAT(4, 9, 416); }                  \
-      else if ((V) == 4) { WHAT(4, 9, 448); }                  \
-      else { WHAT(4, 9, 384); }                                \
-    }                                                          \
-    else {                                                     \
-      if ((V) == 1) { WHAT(2, 33, 128); }                      \
-      else { WHAT(4, 17, 256); }                               \
-    }                                                          \
+    else if ((Nq) <= 16) { WHAT(2, 9, 384); }                  \
+    else if ((Nq) <= 32) { WHAT(4, 9, 384); }                  \
+    else { WHAT(8, 9, 384); }                                  \
   } while (0)
 
 // Fills ctx->cfg_* for ctx->P.Nq (called once by mgrhd_init).
 static cudaError_t configure_ctx(mgrhd_ctx* ctx) {
   cudaError_t e = cudaSuccess;
-  const char* ev = getenv("MGRHD_VARIANT");
-  ctx->variant = ev ? atoi(ev) : 0;
 #define MGRHD_CFG(LL, Q, T) e = Inst<LL, Q, T>::configure(&ctx->cfg_bps); ctx->cfg_l = LL; ctx->cfg_nq = Q; ctx->cfg_threads = T
-  MGRHD_DISPATCH(ctx->P.Nq, ctx->variant, MGRHD_CFG);
+  MGRHD_DISPATCH(ctx->P.Nq, MGRHD_CFG);
 #undef MGRHD_CFG
   if (e == cudaSuccess && ctx->cfg_bps < 1) e = cudaErrorLaunchOutOfResources;
   return e;
@@ -303,7 +293,7 @@ static int launch_update(mgrhd_ctx* ctx, const StatePtrs& S, long long n, long l
   if (blocks > want) blocks = want;
   const bool count = ctx->count_flops != 0;
 #define MGRHD_GO(LL, Q, T) Inst<LL, Q, T>::launch(count, (unsigned)blocks, st, P, S, ctx->d_stats, scratch)
-  MGRHD_DISPATCH(P.Nq, ctx->variant, MGRHD_GO);
+  MGRHD_DISPATCH(P.Nq, MGRHD_GO);
 #undef MGRHD_GO
   ctx->launches++;
   ctx->last_stream = st;

@@ -89,7 +89,7 @@ __device__ __forceinline__ double cell_sum(double v) {
   return v;
 }
 
-// L: lanes that share one cell (1, 2 or 4); lane `sub` of a cell owns edges e = i*L + sub and
+// L: lanes that share one cell (1, 2, 4 or 8); lane `sub` of a cell owns edges e = i*L + sub and
 //    the groups g = e-1 below them, i = 0..NQL-1 ("steps"), so the L lanes of a cell evaluate
 //    NEIGHBOURING edges in the same step (x differs by r_g^(L-1) at most: same branch of
 //    planck_edge almost always) and the lower edge of a group comes from the lane to the left
@@ -120,7 +120,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
   const int tid = threadIdx.x, lane = tid & 31;
   const int sub = lane & (L - 1);                 // position of this lane within its cell
   const unsigned FULL = 0xffffffffu;
-  constexpr unsigned LEADERS = L == 1 ? 0xffffffffu : (L == 2 ? 0x55555555u : 0x11111111u);
+  constexpr unsigned LEADERS = L == 1 ? 0xffffffffu : (L == 2 ? 0x55555555u : (L == 4 ? 0x11111111u : 0x01010101u));
   const int Nq = P.Nq;
   const long long n = P.ncells, stride = P.stride;
   const double dt = P.dt, c = P.c, chat = P.c_hat;
