@@ -114,7 +114,23 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
                      unsigned long long* __restrict__ stats, double* __restrict__ scratch) {
   extern __shared__ double smem[];
   __shared__ unsigned int s_hist[2 * MGRHD_HIST];
+  // Per-edge table rows in shared memory, row e = {nu_e, and for the group below edge e: k_lo, k_hi,
+  // k_mean, 1/k_mean, k_num, 1+alpha, 0}.  The L lanes of a cell read L neighbouring rows per step
+  // (broadcast within equal `sub`), which would otherwise be lane-indexed constant loads that miss
+  // the small indexed-constant cache next to the Planck coefficients (24 % misses measured).
+  __shared__ __align__(16) double s_tab[(kMaxG + 1) * 8];
   for (int t = threadIdx.x; t < 2 * MGRHD_HIST; t += THREADS) s_hist[t] = 0u;
+  for (int r = threadIdx.x; r <= P.Nq; r += THREADS) {
+    const int g = r > 0 ? r - 1 : 0;
+    s_tab[r * 8 + 0] = P.nu[r];
+    s_tab[r * 8 + 1] = P.k_lo[g];
+    s_tab[r * 8 + 2] = P.k_hi[g];
+    s_tab[r * 8 + 3] = P.k_mean[g];
+    s_tab[r * 8 + 4] = P.inv_k_mean[g];
+    s_tab[r * 8 + 5] = P.k_num[g];
+    s_tab[r * 8 + 6] = P.onepa[g];
+    s_tab[r * 8 + 7] = 0.0;
+  }
   __syncthreads();
 
   const int tid = threadIdx.x, lane = tid & 31;
@@ -264,6 +280,10 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
           if (evf) { nF0 = ldd(pF0, oc); nF1 = ldd(pF1, oc); nF2 = ldd(pF2, oc); }
           if (fin) nEo = ldd(pE, of);
         }
+        const double2* const row = reinterpret_cast<const double2*>(&s_tab[(e <= Nq ? e : Nq) * 8]);
+        const double2 r01 = row[0], r23 = row[1], r45 = row[2], r67 = row[3];
+        const double t_nu = r01.x, t_klo = r01.y, t_khi = r23.x, t_kmean = r23.y, t_ikmean = r45.x, t_knum = r45.y,
+                     t_onepa = r67.x;
         const double Rold = sm(SL_R, i);
         // a10 of the cell this lane finished in the previous trip: E_g^(t+1) = E_g^(t) + R_g
         if (fin && vg) *reinterpret_cast<double*>(const_cast<char*>(pE) + of_cur) = Eo + Rold;
@@ -271,8 +291,8 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
         double hi_yz, hi_xi;
         bool hi_small;
         int hf;
-        planck_edge_w(ev && e <= Nq ? P.nu[e <= Nq ? e : Nq] * beta : __longlong_as_double(0x7ff8000000000000ll),
-                      i, hi_yz, hi_xi, hi_small, hf);
+        planck_edge_w(ev && e <= Nq ? t_nu * beta : __longlong_as_double(0x7ff8000000000000ll),
+                      (i & 1) * P.zero, hi_yz, hi_xi, hi_small, hf);
         if (COUNT) eflops += hf;
         double lo_yz, lo_xi;
         bool lo_small;
@@ -296,23 +316,23 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
         // reciprocal is always valid: no slow path, no branch.
         const double dY = hi_small ? hi_yz - lo_yz : (lo_small ? (1.0 - lo_yz) - hi_yz : lo_yz - hi_yz);
         const double dX = hi_xi - lo_xi;
-        const double Dp3 = chis * fma(P.k_hi[gi], hi_xi, -P.k_lo[gi] * lo_xi) * (1.0 / 3.0);
-        const double chiE = chis * P.k_mean[gi];                 // = chi_B (alpha_Q = -1 for both)
+        const double Dp3 = chis * fma(t_khi, hi_xi, -t_klo * lo_xi) * (1.0 / 3.0);
+        const double chiE = chis * t_kmean;                 // = chi_B (alpha_Q = -1 for both)
         const double fbd = fma(4.0, dY, -dX);                    // 3 x denominator of Eq. 27 = T dBt/dT / (a_R T^4)
         // a3: flux-mean opacity, Eq. 27, with the Wien-limit guard (S8)
         const double den = fbd * (1.0 / 3.0);
-        const double num = fma(chis * dY, P.k_num[gi], -Dp3);    // (chi_B + chi_E/3 + alpha chi_E/3) dY - D/3
+        const double num = fma(chis * dY, t_knum, -Dp3);    // (chi_B + chi_E/3 + alpha chi_E/3) dY - D/3
         const bool guard = !(den >= 1e-280) || isinf(aT4 * den);
         double chiF = num * fast_rcp(guard ? 1.0 : den);
-        if (guard) chiF = chis * P.k_lo[gi];
+        if (guard) chiF = chis * t_klo;
         const bool denbad = !(fma(cdt, chiF, 1.0) > 0.0);
         if (denbad) chiF = chiE;
         if (evg && evals == 0) { cnt_guard += guard ? 1u : 0u; cnt_den += denbad ? 1u : 0u; }
         // a4: residuals (Eq. 41; Eq. 42 solved for E_g)
         const double Bt = aT4 * dY;
-        const double inv_chiE = inv_chis * P.inv_k_mean[gi];
-        const double itau = itau_c * P.inv_k_mean[gi];
-        const double W = P.onepa[gi] * chiF * vF * inv_c;
+        const double inv_chiE = inv_chis * t_ikmean;
+        const double itau = itau_c * t_ikmean;
+        const double W = t_onepa * chiF * vF * inv_c;
         const double Eg = fma(W * inv_chiE, inv_c, Bt) - R * itau;
         const double FR = Eg - Et - R;
         // a5: Jacobian (Eq. 44-47) folded into the arrowhead elimination (Eq. 48): 1/J_gg = -q
@@ -403,7 +423,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
         const double Enew = Et + R;                               // E_g^(t+1) = E_g^(t) + R_g
         double p0, p1, p2;
         closure_vP(P.closure, Enew, Fk0, Fk1, Fk2, v0, v1, v2, c, p0, p1, p2);
-        const double w = P.onepa[gi] * (chis * P.k_mean[gi]);     // (1 + alpha) chi_E
+        const double w = s_tab[(gi + 1) * 8 + 6] * (chis * s_tab[(gi + 1) * 8 + 3]);   // (1 + alpha) chi_E
         const double chiF = sm(SL_CHIF, i), A = sm(SL_AG, i);
         const double dn = fma(cdt, chiF, 1.0);                    // 1 + c_hat chi_F dt > 0 (guarded in A)
         const bool dn_ok = dn > 1e-290 && dn < 1e290;
@@ -447,7 +467,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
         const int g = i * L + sub - 1;
         if (fx && g >= 0 && g < Nq) {
           const double vFn = fma(vn0, sm(SL_DA, i), fma(vn1, sm(SL_DB, i), vn2 * sm(SL_AG, i)));
-          const double wf = P.onepa[g] * sm(SL_CHIF, i) * inv_c;
+          const double wf = s_tab[(g + 1) * 8 + 6] * sm(SL_CHIF, i) * inv_c;
           dW += fabs(wf * (vFn - sm(SL_VF, i)));
           sm(SL_VF, i) = vFn;                                       // lagged v.F_g of the next trip
         }

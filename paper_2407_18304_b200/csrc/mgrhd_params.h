@@ -52,6 +52,7 @@ struct Params {
   int Nq;
   int closure;        // 0 Levermore/M1, 1 Eddington
   int newton_maxit, outer_maxit, outer_stop;
+  int zero;           // always 0: an opaque, loop-variant table offset (mgrhd_planck.cuh, planck_edge_w)
   double newton_tol, outer_tol, outer_rel_tol;
   double a_rad;
   double h_over_k;    // h / k_B : x_e = nu_e * h_over_k / T

@@ -145,7 +145,7 @@ __device__ __forceinline__ double2 ld_pair(const Pair& p) { return *reinterpret_
 
 __device__ __forceinline__ void planck_edge_w(double x, int which, double& yz, double& xi, bool& small,
                                               int& flops) {
-  const PlanckTables& tb = mgrhd_c_planck[which & 1];
+  const PlanckTables& tb = mgrhd_c_planck[which];
   const unsigned FULL = 0xffffffffu;
   const bool inS = x < kXS;
   const bool inM = x >= kXS && x < kXL;
