@@ -118,18 +118,19 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
   // k_mean, 1/k_mean, k_num, 1+alpha, 0}.  The L lanes of a cell read L neighbouring rows per step
   // (broadcast within equal `sub`), which would otherwise be lane-indexed constant loads that miss
   // the small indexed-constant cache next to the Planck coefficients (24 % misses measured).
-  __shared__ __align__(16) double s_tab[(kMaxG + 1) * 8];
+  constexpr int TS = 10;   // row stride in doubles: 80 B puts the L rows of a step on distinct banks
+  __shared__ __align__(16) double s_tab[(kMaxG + 1) * TS];
   for (int t = threadIdx.x; t < 2 * MGRHD_HIST; t += THREADS) s_hist[t] = 0u;
   for (int r = threadIdx.x; r <= P.Nq; r += THREADS) {
     const int g = r > 0 ? r - 1 : 0;
-    s_tab[r * 8 + 0] = P.nu[r];
-    s_tab[r * 8 + 1] = P.k_lo[g];
-    s_tab[r * 8 + 2] = P.k_hi[g];
-    s_tab[r * 8 + 3] = P.k_mean[g];
-    s_tab[r * 8 + 4] = P.inv_k_mean[g];
-    s_tab[r * 8 + 5] = P.k_num[g];
-    s_tab[r * 8 + 6] = P.onepa[g];
-    s_tab[r * 8 + 7] = 0.0;
+    s_tab[r * TS + 0] = P.nu[r];
+    s_tab[r * TS + 1] = P.k_lo[g];
+    s_tab[r * TS + 2] = P.k_hi[g];
+    s_tab[r * TS + 3] = P.k_mean[g];
+    s_tab[r * TS + 4] = P.inv_k_mean[g];
+    s_tab[r * TS + 5] = P.k_num[g];
+    s_tab[r * TS + 6] = P.onepa[g];
+    s_tab[r * TS + 7] = 0.0;
   }
   __syncthreads();
 
@@ -280,7 +281,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
           if (evf) { nF0 = ldd(pF0, oc); nF1 = ldd(pF1, oc); nF2 = ldd(pF2, oc); }
           if (fin) nEo = ldd(pE, of);
         }
-        const double2* const row = reinterpret_cast<const double2*>(&s_tab[(e <= Nq ? e : Nq) * 8]);
+        const double2* const row = reinterpret_cast<const double2*>(&s_tab[(e <= Nq ? e : Nq) * TS]);
         const double2 r01 = row[0], r23 = row[1], r45 = row[2], r67 = row[3];
         const double t_nu = r01.x, t_klo = r01.y, t_khi = r23.x, t_kmean = r23.y, t_ikmean = r45.x, t_knum = r45.y,
                      t_onepa = r67.x;
@@ -423,7 +424,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
         const double Enew = Et + R;                               // E_g^(t+1) = E_g^(t) + R_g
         double p0, p1, p2;
         closure_vP(P.closure, Enew, Fk0, Fk1, Fk2, v0, v1, v2, c, p0, p1, p2);
-        const double w = s_tab[(gi + 1) * 8 + 6] * (chis * s_tab[(gi + 1) * 8 + 3]);   // (1 + alpha) chi_E
+        const double w = s_tab[(gi + 1) * TS + 6] * (chis * s_tab[(gi + 1) * TS + 3]);   // (1 + alpha) chi_E
         const double chiF = sm(SL_CHIF, i), A = sm(SL_AG, i);
         const double dn = fma(cdt, chiF, 1.0);                    // 1 + c_hat chi_F dt > 0 (guarded in A)
         const bool dn_ok = dn > 1e-290 && dn < 1e290;
@@ -467,7 +468,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
         const int g = i * L + sub - 1;
         if (fx && g >= 0 && g < Nq) {
           const double vFn = fma(vn0, sm(SL_DA, i), fma(vn1, sm(SL_DB, i), vn2 * sm(SL_AG, i)));
-          const double wf = s_tab[(g + 1) * 8 + 6] * sm(SL_CHIF, i) * inv_c;
+          const double wf = s_tab[(g + 1) * TS + 6] * sm(SL_CHIF, i) * inv_c;
           dW += fabs(wf * (vFn - sm(SL_VF, i)));
           sm(SL_VF, i) = vFn;                                       // lagged v.F_g of the next trip
         }
