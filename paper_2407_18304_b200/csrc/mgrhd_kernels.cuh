@@ -64,11 +64,13 @@ __device__ __forceinline__ void closure_vP(int closure, double E, double F0, dou
   // or f^2 below the normal range (the anisotropic term is then < 1e-290 of the isotropic one)
   const bool iso = closure == 1 || !(E > 0.0) || Fzero || !(f2u > 1e-290);
   const double f2 = f2u > 1.0 ? 1.0 : f2u;
-  const double chi = fma(4.0, f2, 3.0) * fast_rcp(fma(2.0, sqrt(fma(-3.0, f2, 4.0)), 5.0));
+  // chi = (3 + 4 f^2)/(5 + 2 s), s = sqrt(4 - 3 f^2), equals (5 - 2 s)/3 (multiply through by 5 - 2 s), so
+  // (1 - chi)/2 = (s - 1)/3 and (3 chi - 1)/2 = 2 - s: one sqrt, no division
+  const double sq = sqrt(fma(-3.0, f2, 4.0));
   const double r2 = fast_rcp(iso || !(f2u < 1e290) ? 1.0 : f2u);
   const double tv = fma(t0, v0, fma(t1, v1, t2 * v2));
-  const double a = iso ? 1.0 / 3.0 : 0.5 * (1.0 - chi);
-  const double b = 0.5 * fma(3.0, chi, -1.0) * tv * r2;
+  const double a = iso ? 1.0 / 3.0 : (sq - 1.0) * (1.0 / 3.0);
+  const double b = (2.0 - sq) * tv * r2;
   p0 = E * fma(a, v0, iso ? 0.0 : b * t0);       // (t may be inf/NaN on isotropic lanes: selected away)
   p1 = E * fma(a, v1, iso ? 0.0 : b * t1);
   p2 = E * fma(a, v2, iso ? 0.0 : b * t2);
@@ -147,8 +149,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
   const long long tthreads = (long long)gridDim.x * THREADS;
   const long long gtid = (long long)blockIdx.x * THREADS + tid;
   auto sm = [&](int s, int i) -> double& { return smem[(s * NQL + i) * THREADS + tid]; };
-  // F_g^(t), component k, step i of this lane (global scratch, coalesced across the warp)
-  auto ft = [&](int k, int i) -> double& { return scratch[(long long)(k * NQL + i) * tthreads + gtid]; };
+  // scratch: F_g^(t), component k, step i of this lane at scratch[(k*NQL + i)*tthreads + gtid] (coalesced)
 
   // this warp's contiguous chunk of cells [next, end)
   const long long nwarps = tthreads >> 5, wid = gtid >> 5;
@@ -400,11 +401,13 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
       const long long dstep = (long long)L * stride * 8;
       long long oc = ((long long)(sub - 1) * stride + cell) * 8, oc_cur = oc;
       auto ldd = [](const char* p, long long o) { return *reinterpret_cast<const double*>(p + o); };
+      double* ftp = scratch + gtid;                    // F_g^(t) scratch of this lane: step i at ftp, components ftc apart
+      const long long ftc = (long long)NQL * tthreads;
       double nEt = 0.0, nFt0 = 0.0, nFt1 = 0.0, nFt2 = 0.0, nFk0 = 0.0, nFk1 = 0.0, nFk2 = 0.0;
       if (fx && sub >= 1 && sub - 1 < Nq) {
         nEt = ldd(pE, oc);
         nFk0 = ldd(pF0, oc); nFk1 = ldd(pF1, oc); nFk2 = ldd(pF2, oc);
-        if (!t0) { nFt0 = ft(0, 0); nFt1 = ft(1, 0); nFt2 = ft(2, 0); }
+        if (!t0) { nFt0 = ftp[0]; nFt1 = ftp[ftc]; nFt2 = ftp[2 * ftc]; }
       }
 #pragma unroll 1
       for (int i = 0; i < NQL; ++i) {      // executed by all lanes with per-lane predicates, like loop A
@@ -418,7 +421,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
         if (fx && g + L >= 0 && g + L < Nq) {
           nEt = ldd(pE, oc);
           nFk0 = ldd(pF0, oc); nFk1 = ldd(pF1, oc); nFk2 = ldd(pF2, oc);
-          if (!t0) { nFt0 = ft(0, i + 1); nFt1 = ft(1, i + 1); nFt2 = ft(2, i + 1); }
+          if (!t0) { nFt0 = ftp[tthreads]; nFt1 = ftp[tthreads + ftc]; nFt2 = ftp[tthreads + 2 * ftc]; }
         }
         const double R = sm(SL_R, i);
         const double Enew = Et + R;                               // E_g^(t+1) = E_g^(t) + R_g
@@ -446,13 +449,14 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
           sumAbsR += fabs(R);
           dF0 += Fn0 - Ft0; dF1 += Fn1 - Ft1; dF2 += Fn2 - Ft2;
           if (P.outer_stop == 1 && !ok) rel_bad = 1;
-          if (t0) { ft(0, i) = Ft0; ft(1, i) = Ft1; ft(2, i) = Ft2; }
+          if (t0) { ftp[0] = Ft0; ftp[ftc] = Ft1; ftp[2 * ftc] = Ft2; }
           // lagged flux of the next trip, in place
           *reinterpret_cast<double*>(pF0 + oc_cur) = Fn0;
           *reinterpret_cast<double*>(pF1 + oc_cur) = Fn1;
           *reinterpret_cast<double*>(pF2 + oc_cur) = Fn2;
           sm(SL_DA, i) = Fn0; sm(SL_DB, i) = Fn1; sm(SL_AG, i) = Fn2;   // kept on chip for loop C
         }
+        ftp += tthreads;
       }
       sumR = cell_sum<L>(sumR); sumAbsR = cell_sum<L>(sumAbsR);
       dF0 = cell_sum<L>(dF0); dF1 = cell_sum<L>(dF1); dF2 = cell_sum<L>(dF2);

@@ -43,7 +43,7 @@ constexpr int kFlopCellEval = 24;     // T, a_R T^4, beta, scales, v, F_G, Eq. 4
 constexpr int kFlopStepCell = 10;     // dx0, T > 0 check, E_gas update
 constexpr int kFlopStepGroup = 4;     // R_g += lam da_g + (lam dx0) db_g
 constexpr int kFlopOuterCell = 50;    // v, Eq. 52, commit, E_kin, outer tests, sums over the cell's lanes
-constexpr int kFlopOuterGroup = 109;  // closure (53), Eq. 51 (23), relative-change test (14), sums (9), next v.F_g and dW (10)
+constexpr int kFlopOuterGroup = 102;  // closure (46), Eq. 51 (23), relative-change test (14), sums (9), next v.F_g and dW (10)
 constexpr int kFlopCell = 16;         // load-time derivations
 constexpr int kFlopCellGroup = 7;     // sum E_g, first v.F_g, E_g commit
 
