@@ -117,7 +117,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
   extern __shared__ double smem[];
   __shared__ unsigned int s_hist[2 * MGRHD_HIST];
   // Per-edge table rows in shared memory, row e = {nu_e, and for the group below edge e: k_lo, k_hi,
-  // k_mean, 1/k_mean, k_num, 1+alpha, 0}.  The L lanes of a cell read L neighbouring rows per step
+  // k_mean, 1/k_mean, (4+alpha) k_mean, 1+alpha, (1+alpha)/k_mean}.  The L lanes of a cell read L neighbouring rows per step
   // (broadcast within equal `sub`), which would otherwise be lane-indexed constant loads that miss
   // the small indexed-constant cache next to the Planck coefficients (24 % misses measured).
   constexpr int TS = 10;   // row stride in doubles: 80 B puts the L rows of a step on distinct banks
@@ -130,9 +130,9 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
     s_tab[r * TS + 2] = P.k_hi[g];
     s_tab[r * TS + 3] = P.k_mean[g];
     s_tab[r * TS + 4] = P.inv_k_mean[g];
-    s_tab[r * TS + 5] = P.k_num[g];
+    s_tab[r * TS + 5] = 3.0 * P.k_num[g];                  // (4 + alpha) k_mean
     s_tab[r * TS + 6] = P.onepa[g];
-    s_tab[r * TS + 7] = 0.0;
+    s_tab[r * TS + 7] = P.onepa[g] * P.inv_k_mean[g];      // (1 + alpha)/k_mean
   }
   __syncthreads();
 
@@ -236,7 +236,9 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
       const double aT4 = P.a_rad * T2 * T2;
       const double beta = P.h_over_k * invT;
       const double itau_c = inv_chis / cdt;          // 1/(c_hat dt chi_E,g) = itau_c * inv_k_mean[g]
-      const double dBscale = invT * inv_Cv;          // J_g0 = (4 Bt - Db) / (T C_v), Eq. 46
+      const double jscale = aT4 * invT * inv_Cv;     // J_g0 = (4 Bt - Db) / (T C_v), Eq. 46, per unit (4 dY - dXi)
+      const double wscale = inv_chis * inv_c * inv_c; // W_g/(c chi_E) = (1+alpha)/k_mean chi_F v.F wscale
+      const double agscale = aT4 * chis;
       const double v0 = momk0 * inv_rho, v1 = momk1 * inv_rho, v2 = momk2 * inv_rho;
       double sumR = 0.0, sumAbsFR = 0.0, SFRq = 0.0, SJq = 0.0, sumEt = 0.0;
       int eflops = 0;
@@ -284,8 +286,8 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
         }
         const double2* const row = reinterpret_cast<const double2*>(&s_tab[(e <= Nq ? e : Nq) * TS]);
         const double2 r01 = row[0], r23 = row[1], r45 = row[2], r67 = row[3];
-        const double t_nu = r01.x, t_klo = r01.y, t_khi = r23.x, t_kmean = r23.y, t_ikmean = r45.x, t_knum = r45.y,
-                     t_onepa = r67.x;
+        const double t_nu = r01.x, t_klo = r01.y, t_khi = r23.x, t_kmean = r23.y, t_ikmean = r45.x, t_knum3 = r45.y,
+                     t_wc = r67.y;
         const double Rold = sm(SL_R, i);
         // a10 of the cell this lane finished in the previous trip: E_g^(t+1) = E_g^(t) + R_g
         if (fin && vg) *reinterpret_cast<double*>(const_cast<char*>(pE) + of_cur) = Eo + Rold;
@@ -318,28 +320,24 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
         // reciprocal is always valid: no slow path, no branch.
         const double dY = hi_small ? hi_yz - lo_yz : (lo_small ? (1.0 - lo_yz) - hi_yz : lo_yz - hi_yz);
         const double dX = hi_xi - lo_xi;
-        const double Dp3 = chis * fma(t_khi, hi_xi, -t_klo * lo_xi) * (1.0 / 3.0);
-        const double chiE = chis * t_kmean;                 // = chi_B (alpha_Q = -1 for both)
+        const double P3 = fma(t_khi, hi_xi, -t_klo * lo_xi);     // Delta_g(nu chi_0 B_nu) per unit chis a_R T^4
         const double fbd = fma(4.0, dY, -dX);                    // 3 x denominator of Eq. 27 = T dBt/dT / (a_R T^4)
-        // a3: flux-mean opacity, Eq. 27, with the Wien-limit guard (S8)
-        const double den = fbd * (1.0 / 3.0);
-        const double num = fma(chis * dY, t_knum, -Dp3);    // (chi_B + chi_E/3 + alpha chi_E/3) dY - D/3
-        const bool guard = !(den >= 1e-280) || isinf(aT4 * den);
-        double chiF = num * fast_rcp(guard ? 1.0 : den);
+        // a3: flux-mean opacity, Eq. 27 x 3/3: chi_F = chis ((4+alpha) k_mean dY - P3) / (4 dY - dXi),
+        //     with the Wien-limit guard (S8)
+        const bool guard = !(fbd >= 3e-280) || isinf(aT4 * fbd);
+        double chiF = chis * (fma(t_knum3, dY, -P3) * fast_rcp(guard ? 1.0 : fbd));
         if (guard) chiF = chis * t_klo;
         const bool denbad = !(fma(cdt, chiF, 1.0) > 0.0);
-        if (denbad) chiF = chiE;
+        if (denbad) chiF = chis * t_kmean;
         if (evg && evals == 0) { cnt_guard += guard ? 1u : 0u; cnt_den += denbad ? 1u : 0u; }
-        // a4: residuals (Eq. 41; Eq. 42 solved for E_g)
-        const double Bt = aT4 * dY;
-        const double inv_chiE = inv_chis * t_ikmean;
-        const double itau = itau_c * t_ikmean;
-        const double W = t_onepa * chiF * vF * inv_c;
-        const double Eg = fma(W * inv_chiE, inv_c, Bt) - R * itau;
-        const double FR = Eg - Et - R;
+        // a4: residuals (Eq. 41; Eq. 42 solved for E_g):
+        //     F_R,g = Bt + W_g/(c chi_E) - E_g^t - R_g (1 + 1/(c_hat dt chi_E))
+        const double opi = fma(itau_c, t_ikmean, 1.0);           // 1 + 1/(c_hat dt chi_E) = -J_gg (Eq. 47)
+        const double Wc = (chiF * vF) * (t_wc * wscale);         // (1+alpha) chi_F v.F / (c^2 chi_E)
+        const double FR = fma(-R, opi, fma(aT4, dY, Wc) - Et);
         // a5: Jacobian (Eq. 44-47) folded into the arrowhead elimination (Eq. 48): 1/J_gg = -q
-        const double q = fast_rcp(1.0 + itau);
-        const double da = FR * q, db = aT4 * fbd * dBscale * q;
+        const double q = fast_rcp(opi);
+        const double da = FR * q, db = (fbd * q) * jscale;
         if (evg) {
           sumR += R;
           sumAbsFR += fabs(FR);
@@ -347,7 +345,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
           SJq += db;
           sm(SL_DA, i) = da;
           sm(SL_DB, i) = db;
-          sm(SL_AG, i) = aT4 * fma(chiE, dY, -Dp3);              // chi_B Bt - D/3 (Eq. 51 source)
+          sm(SL_AG, i) = agscale * fma(t_kmean, dY, P3 * (-1.0 / 3.0));   // chi_B Bt - D/3 (Eq. 51 source)
           sm(SL_CHIF, i) = chiF;
         }
       }

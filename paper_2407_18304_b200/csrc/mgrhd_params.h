@@ -38,8 +38,8 @@ constexpr int kFlopEdgeSmall = 59;    // x < kXS: x, x^2, two 12-term Horner cha
 constexpr int kFlopEdgeMid = 95;      // kXS <= x < kXL: x, t, two degree-23 Horner chains
 constexpr int kFlopEdgeLarge = 96;    // x >= kXL: x, exp, 7 terms of (3+1) FMA, Xi with one reciprocal
 constexpr int kFlopEdgeZero = 32;     // x, exp that underflowed
-constexpr int kFlopGroupEval = 47;    // a2-a5 for one group at one trial T
-constexpr int kFlopCellEval = 24;     // T, a_R T^4, beta, scales, v, F_G, Eq. 49, sums over the cell's lanes
+constexpr int kFlopGroupEval = 39;    // a2-a5 for one group at one trial T
+constexpr int kFlopCellEval = 27;     // T, a_R T^4, beta, scales, v, F_G, Eq. 49, sums over the cell's lanes
 constexpr int kFlopStepCell = 10;     // dx0, T > 0 check, E_gas update
 constexpr int kFlopStepGroup = 4;     // R_g += lam da_g + (lam dx0) db_g
 constexpr int kFlopOuterCell = 50;    // v, Eq. 52, commit, E_kin, outer tests, sums over the cell's lanes
