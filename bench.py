@@ -326,10 +326,10 @@ def run_ours(args) -> None:
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the update kernel, from the
-# `ncu --set full` capture summarised in profiles/r1_v9_ncu_full.md: 2.683 + 6.095 GB at
+# `ncu --set full` capture summarised in profiles/r1_final_ncu_full.md: 2.678 + 6.115 GB at
 # 2 097 152 cells of config 4, scaled x8 to its 16 777 216 cells (persistent grid-stride kernel,
 # traffic linear in cells).  None for workloads without a capture.
-NCU_TRAFFIC_BYTES: dict = {4: 8.0 * (2.682634e9 + 6.095024e9)}
+NCU_TRAFFIC_BYTES: dict = {4: 8.0 * (2.677987e9 + 6.114892e9)}
 
 
 def run_e2e(args, wl, ctx, pristine, dt, world, dist):
