@@ -436,7 +436,7 @@ int mgrhd_planck_edge_functions(const double* x_dev, long long n, double* yz_dev
   CU(upload_tables_for_current_device());
   long long blocks = (n + 255) / 256;
   if (blocks > 4096) blocks = 4096;
-  planck_edge_kernel<<<(unsigned)blocks, 256, 0, (cudaStream_t)stream>>>(x_dev, n, yz_dev, xi_dev, is_y_dev);
+  planck_edge_kernel<<<(unsigned)blocks, 256, 0, (cudaStream_t)stream>>>(x_dev, n, yz_dev, xi_dev, is_y_dev, 0);
   CU(cudaGetLastError());
   return MGRHD_OK;
 }

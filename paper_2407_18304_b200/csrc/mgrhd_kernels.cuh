@@ -35,12 +35,6 @@ __device__ __forceinline__ double fast_rcp(double x) {   // declared in mgrhd_pl
   return r;
 }
 
-// L1 prefetch of one global address (no register, no dependency)
-__device__ __forceinline__ void prefetch_l1(const double* p) {
-  asm volatile("prefetch.global.L1 [%0];" ::"l"(p));
-}
-constexpr int kPrefetchDist = 4;   // groups ahead
-
 __device__ __forceinline__ double norm3(double a, double b, double c) {
   return sqrt(fma(a, a, fma(b, b, c * c)));
 }
@@ -558,15 +552,23 @@ __global__ void conserved_totals_kernel(const __grid_constant__ StatePtrs S, int
   }
 }
 
-// Diagnostic: the edge functions on an array of x (tests pin them against the oracle's).
+// Diagnostic: the edge functions (the very planck_edge_w the update kernel uses) on an array of x;
+// tests pin them against the oracle's.  Whole warps run the loop so the warp-converged branches
+// see all 32 lanes; lanes past the end pass NaN (no branch) and store nothing.
 __global__ void planck_edge_kernel(const double* __restrict__ x, long long n, double* __restrict__ yz,
-                                   double* __restrict__ xi, int* __restrict__ is_y) {
-  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n;
+                                   double* __restrict__ xi, int* __restrict__ is_y, int zero) {
+  const long long nround = (n + 31) / 32 * 32;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < nround;
        i += (long long)gridDim.x * blockDim.x) {
-    const EdgeFn e = planck_edge(x[i], planck_table_base((int)(i & 1)));
-    yz[i] = e.yz;
-    xi[i] = e.xi;
-    is_y[i] = e.small ? 1 : 0;
+    double a, b;
+    bool small;
+    int fl;
+    planck_edge_w(i < n ? x[i] : __longlong_as_double(0x7ff8000000000000ll), (int)(i & 1) * zero, a, b, small, fl);
+    if (i < n) {
+      yz[i] = a;
+      xi[i] = b;
+      is_y[i] = small ? 1 : 0;
+    }
   }
 }
 
