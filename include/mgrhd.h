@@ -101,7 +101,9 @@ int mgrhd_init(mgrhd_ctx **out, const double *group_edges, int Nq,
  * (PAPER.md:389), speed of light c and reduced speed of light c_hat <= c (Eq. 34).
  * Stream-ordered on `cuda_stream` (a cudaStream_t, NULL = default stream), asynchronous:
  * no host synchronisation, no allocation.  ncells == 0 is a no-op.  Per-cell numerical
- * failures never abort; they are counted in mgrhd_stats. */
+ * failures never abort; they are counted in mgrhd_stats.  A context owns one scratch buffer:
+ * at most ONE mgrhd_source_update per context may be in flight at a time (calls on the same
+ * stream are naturally serialised; use one context per stream for concurrent updates). */
 int mgrhd_source_update(mgrhd_ctx *ctx, const mgrhd_state *state_dev, long long ncells,
                         double dt, double c, double c_hat, void *cuda_stream);
 

@@ -268,7 +268,6 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
         const int g = e - 1;                         // group below it
         const bool vg = g >= 0 && g < Nq;
         const bool evg = ev && vg;
-        const int gi = vg ? g : 0;                   // safe table index
         const double Et = nEt, F0 = nF0, F1 = nF1, F2 = nF2, Eo = nEo;
         of_cur = of;
         oc += dstep;
