@@ -35,6 +35,15 @@ __device__ __forceinline__ double fast_rcp(double x) {   // declared in mgrhd_pl
   return r;
 }
 
+// 1/x for a converged warp: the fast reciprocal, with IEEE division only when some lane's |x| is
+// outside [1e-290, 1e290] (a warp-uniform, practically never taken branch).
+__device__ __forceinline__ double warp_rcp(double x) {
+  const bool ok = fabs(x) > 1e-290 && fabs(x) < 1e290;
+  double r = fast_rcp(ok ? x : 1.0);
+  if (__any_sync(0xffffffffu, !ok)) r = ok ? r : 1.0 / x;
+  return r;
+}
+
 __device__ __forceinline__ double norm3(double a, double b, double c) {
   return sqrt(fma(a, a, fma(b, b, c * c)));
 }
@@ -137,7 +146,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
   const int Nq = P.Nq;
   const long long n = P.ncells, stride = P.stride;
   const double dt = P.dt, c = P.c, chat = P.c_hat;
-  const double c_over_chat = c / chat, inv_c = 1.0 / c, cdt = chat * dt, icc = 1.0 / (c * chat);
+  const double c_over_chat = c / chat, inv_c = 1.0 / c, cdt = chat * dt, icc = 1.0 / (c * chat), inv_cdt = 1.0 / cdt;
   const double rel2 = P.outer_rel_tol * P.outer_rel_tol;
 
   const long long tthreads = (long long)gridDim.x * THREADS;
@@ -225,11 +234,11 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
       const bool ev = phase == PH_EVAL;
       const bool fin = fin_cell >= 0;
       const double T = ev ? (Egs - Ekin) * inv_Cv : 1.0;
-      const double invT = 1.0 / T;
+      const double invT = warp_rcp(T);
       const double T2 = T * T;
       const double aT4 = P.a_rad * T2 * T2;
       const double beta = P.h_over_k * invT;
-      const double itau_c = inv_chis / cdt;          // 1/(c_hat dt chi_E,g) = itau_c * inv_k_mean[g]
+      const double itau_c = inv_chis * inv_cdt;         // 1/(c_hat dt chi_E,g) = itau_c * inv_k_mean[g]
       const double jscale = aT4 * invT * inv_Cv;     // J_g0 = (4 Bt - Db) / (T C_v), Eq. 46, per unit (4 dY - dXi)
       const double wscale = inv_chis * inv_c * inv_c; // W_g/(c chi_E) = (1+alpha)/k_mean chi_F v.F wscale
       const double agscale = aT4 * chis;
@@ -348,14 +357,19 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
       SFRq = cell_sum<L>(SFRq); SJq = cell_sum<L>(SJq);
       if (__any_sync(FULL, ev && first)) sumEt = cell_sum<L>(sumEt);
       if (COUNT && ev) flops += (unsigned)eflops + (sub == 0 ? kFlopCellEval + kFlopGroupEval * Nq : 0);
+      // 1/(1 - sum J0g Jg0/Jgg) of the gas-row elimination (>= 1 for any physical state), formed warp-wide
+      const double inv_jd = warp_rcp(fma(c_over_chat, SJq, 1.0));
       if (ev) {
         if (first) Etot = Egas_t + (chat / c) * sumEt;             // Eq. 50 as printed, S_g = 0
         first = false;
         pend = false;
         const double FG = Egs - Egas_t + c_over_chat * sumR;
         evals++;
-        const double inv_Etot = 1.0 / Etot;
-        if (fabs(FG) * inv_Etot < P.newton_tol && c_over_chat * sumAbsFR * inv_Etot < P.newton_tol) {
+        // Eq. 49 (|F_G|/E_tot < eps and (c/c_hat) sum|F_R|/E_tot < eps), without the divisions for E_tot > 0
+        const bool conv = Etot > 0.0
+            ? (fabs(FG) < P.newton_tol * Etot && c_over_chat * sumAbsFR < P.newton_tol * Etot)
+            : (fabs(FG) / Etot < P.newton_tol && c_over_chat * sumAbsFR / Etot < P.newton_tol);
+        if (conv) {
           phase = PH_FLUX;                                          // Eq. 49 met
         } else if (it >= P.newton_maxit) {
           if (sub == 0) cnt_newton_unconv++;
@@ -363,7 +377,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
         } else {
           // Newton step: eliminate the gas row
           //   dx0 = (-F_G + sum J0g F_R,g/Jgg) / (1 - sum J0g Jg0/Jgg),  dR_g = (F_R,g + Jg0 dx0) q
-          const double dx0 = (-FG - c_over_chat * SFRq) / fma(c_over_chat, SJq, 1.0);
+          const double dx0 = (-FG - c_over_chat * SFRq) * inv_jd;
           lam = 1.0;
           for (int h = 0; h < 10 && !((Egs + lam * dx0 - Ekin) * inv_Cv > 0.0); ++h) {
             lam *= 0.5;
