@@ -157,7 +157,7 @@ struct mgrhd_ctx {
 // with as many threads per SM as the register file allows.
 template <int L, int NQL, int THREADS>
 struct Inst {
-  static constexpr size_t kSmem = (size_t)SL_COUNT * NQL * THREADS * sizeof(double);
+  static constexpr size_t kSmem = ((size_t)SL_COUNT * NQL + 1) * THREADS * sizeof(double);   // + one padding row
   static cudaError_t configure(int* blocks_per_sm) {
     cudaError_t e = cudaFuncSetAttribute(source_update_kernel<L, NQL, THREADS, false>,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem);

@@ -101,7 +101,7 @@ __device__ __forceinline__ double cell_sum(double v) {
 //    by one shuffle.  A warp works on 32/L cells at a time; per-thread state shrinks by L, so
 //    L times more threads fit beside the same shared memory.
 // NQL: steps per lane, NQL*L >= Nq+1.   THREADS: CTA size.
-// Dynamic shared memory: SL_COUNT * NQL * THREADS doubles, laid out [slot][step][thread].
+// Dynamic shared memory: (SL_COUNT * NQL + 1) * THREADS doubles: one padding row, then [slot][step][thread].
 // scratch: 3 * NQL * (gridDim.x*THREADS) doubles of global memory, private to this launch:
 //    F_g^(t) of the cell in flight (the state's Frad holds the lagged F_g,k in place).
 //
@@ -117,7 +117,8 @@ template <int L, int NQL, int THREADS, bool COUNT>
 __global__ void __launch_bounds__(THREADS, 1)
 source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ StatePtrs S,
                      unsigned long long* __restrict__ stats, double* __restrict__ scratch) {
-  extern __shared__ double smem[];
+  extern __shared__ double smem_raw[];
+  double* const smem = smem_raw + THREADS;   // one row of padding: loop A's shifted column of step 0 stays in bounds
   __shared__ unsigned int s_hist[2 * MGRHD_HIST];
   // Per-edge table rows in shared memory, row e = {nu_e, and for the group below edge e: k_lo, k_hi,
   // k_mean, 1/k_mean, (4+alpha) k_mean, 1+alpha, (1+alpha)/k_mean}.  The L lanes of a cell read L neighbouring rows per step
@@ -151,7 +152,14 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
 
   const long long tthreads = (long long)gridDim.x * THREADS;
   const long long gtid = (long long)blockIdx.x * THREADS + tid;
-  auto sm = [&](int s, int i) -> double& { return smem[(s * NQL + i) * THREADS + tid]; };
+  // Per-group values live in shared memory in GROUP order: group g at step g/L of lane g%L of its
+  // cell (smG), so the flux loops B and C take ceil(Nq/L) full steps.  Loop A walks EDGES
+  // (e = i*L + sub, group g = e - 1): its group sits one lane to the left, or for sub == 0 in the
+  // previous step of the cell's last lane -- a fixed per-lane offset (smA).
+  const int shiftA = sub ? -1 : (L - 1) - THREADS;
+  auto smG = [&](int s, int i) -> double& { return smem[(s * NQL + i) * THREADS + tid]; };
+  auto sm = [&](int s, int i) -> double& { return smem[(s * NQL + i) * THREADS + tid + shiftA]; };
+  const int NG = (Nq + L - 1) / L;                 // steps of the flux loops
   // scratch: F_g^(t), component k, step i of this lane at scratch[(k*NQL + i)*tthreads + gtid] (coalesced)
 
   // this warp's contiguous chunk of cells [next, end)
@@ -231,6 +239,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
 
     // ===== A: all edges/groups at the trial temperature (a1-a5), then Eq. 49 =======================
     if (__any_sync(FULL, phase == PH_EVAL)) {
+      __syncwarp();        // loop C's v.F_g (group order) is read through the shifted column
       const bool ev = phase == PH_EVAL;
       const bool fin = fin_cell >= 0;
       const double T = ev ? (Egs - Ekin) * inv_Cv : 1.0;
@@ -394,6 +403,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
 
     // ===== B, C: energy commit (a6), closure + Eq. 51 (a7), Eq. 52 (a8), outer test (a9) ==========
     if (__any_sync(FULL, phase == PH_FLUX)) {
+      __syncwarp();        // loop A wrote R_g, chi_F, A_g through the shifted column
       const bool fx = phase == PH_FLUX;
       const bool t0 = trips == 0;       // first trip: F_g^(t) is still in the state, save it to the scratch
       const double v0 = momk0 * inv_rho, v1 = momk1 * inv_rho, v2 = momk2 * inv_rho;
@@ -404,36 +414,36 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
       char* const pF1 = reinterpret_cast<char*>(S.Frad[1]);
       char* const pF2 = reinterpret_cast<char*>(S.Frad[2]);
       const long long dstep = (long long)L * stride * 8;
-      long long oc = ((long long)(sub - 1) * stride + cell) * 8, oc_cur = oc;
+      long long oc = ((long long)sub * stride + cell) * 8, oc_cur = oc;      // group g = i*L + sub
       auto ldd = [](const char* p, long long o) { return *reinterpret_cast<const double*>(p + o); };
       double* ftp = scratch + gtid;                    // F_g^(t) scratch of this lane: step i at ftp, components ftc apart
       const long long ftc = (long long)NQL * tthreads;
       double nEt = 0.0, nFt0 = 0.0, nFt1 = 0.0, nFt2 = 0.0, nFk0 = 0.0, nFk1 = 0.0, nFk2 = 0.0;
-      if (fx && sub >= 1 && sub - 1 < Nq) {
+      if (fx && sub < Nq) {
         nEt = ldd(pE, oc);
         nFk0 = ldd(pF0, oc); nFk1 = ldd(pF1, oc); nFk2 = ldd(pF2, oc);
         if (!t0) { nFt0 = ftp[0]; nFt1 = ftp[ftc]; nFt2 = ftp[2 * ftc]; }
       }
 #pragma unroll 1
-      for (int i = 0; i < NQL; ++i) {      // executed by all lanes with per-lane predicates, like loop A
-        const int g = i * L + sub - 1;
-        const bool vg = fx && g >= 0 && g < Nq;
-        const int gi = g >= 0 && g < Nq ? g : 0;
+      for (int i = 0; i < NG; ++i) {       // executed by all lanes with per-lane predicates, like loop A
+        const int g = i * L + sub;
+        const bool vg = fx && g < Nq;
+        const int gi = g < Nq ? g : 0;
         const double Et = nEt, Fk0 = nFk0, Fk1 = nFk1, Fk2 = nFk2;
         const double Ft0 = t0 ? nFk0 : nFt0, Ft1 = t0 ? nFk1 : nFt1, Ft2 = t0 ? nFk2 : nFt2;
         oc_cur = oc;
         oc += dstep;
-        if (fx && g + L >= 0 && g + L < Nq) {
+        if (fx && g + L < Nq) {
           nEt = ldd(pE, oc);
           nFk0 = ldd(pF0, oc); nFk1 = ldd(pF1, oc); nFk2 = ldd(pF2, oc);
           if (!t0) { nFt0 = ftp[tthreads]; nFt1 = ftp[tthreads + ftc]; nFt2 = ftp[tthreads + 2 * ftc]; }
         }
-        const double R = sm(SL_R, i);
+        const double R = smG(SL_R, i);
         const double Enew = Et + R;                               // E_g^(t+1) = E_g^(t) + R_g
         double p0, p1, p2;
         closure_vP(P.closure, Enew, Fk0, Fk1, Fk2, v0, v1, v2, c, p0, p1, p2);
         const double w = s_tab[(gi + 1) * TS + 6] * (chis * s_tab[(gi + 1) * TS + 3]);   // (1 + alpha) chi_E
-        const double chiF = sm(SL_CHIF, i), A = sm(SL_AG, i);
+        const double chiF = smG(SL_CHIF, i), A = smG(SL_AG, i);
         const double dn = fma(cdt, chiF, 1.0);                    // 1 + c_hat chi_F dt > 0 (guarded in A)
         const bool dn_ok = dn > 1e-290 && dn < 1e290;
         double inv_dn = fast_rcp(dn_ok ? dn : 1.0);
@@ -459,7 +469,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
           *reinterpret_cast<double*>(pF0 + oc_cur) = Fn0;
           *reinterpret_cast<double*>(pF1 + oc_cur) = Fn1;
           *reinterpret_cast<double*>(pF2 + oc_cur) = Fn2;
-          sm(SL_DA, i) = Fn0; sm(SL_DB, i) = Fn1; sm(SL_AG, i) = Fn2;   // kept on chip for loop C
+          smG(SL_DA, i) = Fn0; smG(SL_DB, i) = Fn1; smG(SL_AG, i) = Fn2;   // kept on chip for loop C
         }
         ftp += tthreads;
       }
@@ -473,13 +483,13 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
       }
       const double vn0 = momn0 * inv_rho, vn1 = momn1 * inv_rho, vn2 = momn2 * inv_rho;
 #pragma unroll 1
-      for (int i = 0; i < NQL; ++i) {
-        const int g = i * L + sub - 1;
-        if (fx && g >= 0 && g < Nq) {
-          const double vFn = fma(vn0, sm(SL_DA, i), fma(vn1, sm(SL_DB, i), vn2 * sm(SL_AG, i)));
-          const double wf = s_tab[(g + 1) * TS + 6] * sm(SL_CHIF, i) * inv_c;
-          dW += fabs(wf * (vFn - sm(SL_VF, i)));
-          sm(SL_VF, i) = vFn;                                       // lagged v.F_g of the next trip
+      for (int i = 0; i < NG; ++i) {
+        const int g = i * L + sub;
+        if (fx && g < Nq) {
+          const double vFn = fma(vn0, smG(SL_DA, i), fma(vn1, smG(SL_DB, i), vn2 * smG(SL_AG, i)));
+          const double wf = s_tab[(g + 1) * TS + 6] * smG(SL_CHIF, i) * inv_c;
+          dW += fabs(wf * (vFn - smG(SL_VF, i)));
+          smG(SL_VF, i) = vFn;                                       // lagged v.F_g of the next trip
         }
       }
       dW = cell_sum<L>(dW);
@@ -517,12 +527,13 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
   }
 
   // E_g store of the last cell of each lane (no further loop A ran for it)
+  __syncwarp();
   if (fin_cell >= 0)
-    for (int i = 0; i < NQL; ++i) {
-      const int g = i * L + sub - 1;
-      if (g >= 0 && g < Nq) {
+    for (int i = 0; i < NG; ++i) {
+      const int g = i * L + sub;
+      if (g < Nq) {
         const long long o = (long long)g * stride + fin_cell;
-        S.Erad[o] = S.Erad[o] + sm(SL_R, i);
+        S.Erad[o] = S.Erad[o] + smG(SL_R, i);
       }
     }
 
