@@ -404,46 +404,80 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
     // ===== B, C: energy commit (a6), closure + Eq. 51 (a7), Eq. 52 (a8), outer test (a9) ==========
     if (__any_sync(FULL, phase == PH_FLUX)) {
       __syncwarp();        // loop A wrote R_g, chi_F, A_g through the shifted column
-      const bool fx = phase == PH_FLUX;
-      const bool t0 = trips == 0;       // first trip: F_g^(t) is still in the state, save it to the scratch
-      const double v0 = momk0 * inv_rho, v1 = momk1 * inv_rho, v2 = momk2 * inv_rho;
+      const bool fxo = phase == PH_FLUX;      // this lane's own cell is in the flux phase
+      // Lane assignment of this pass.  Only the w cells in the flux phase have work here (a bit more
+      // than half of the warp's cells on average), so the groups of each are spread over LB = L*kS
+      // lanes, kS the largest power of two with w*LB <= 32: block j of LB lanes works for the j-th
+      // flux cell ("owner"), reads its scalars by shuffle and its per-group columns in shared memory
+      // and in the scratch directly, and hands the sums back.  kS = 1 is the plain case: every lane
+      // works for its own cell.
+      constexpr int LOG2L = L == 1 ? 0 : (L == 2 ? 1 : (L == 4 ? 2 : 3));
+      const unsigned fm = __ballot_sync(FULL, fxo) & LEADERS;
+      const int w = __popc(fm);
+      int ksh = 0;
+      while (((w * L) << (ksh + 1)) <= 32) ++ksh;
+      const int lsh = ksh + LOG2L, LB = 1 << lsh;
+      const int subB = lane & (LB - 1), j = lane >> lsh;
+      const bool fx = ksh ? j < w : fxo;
+      const int own = ksh ? (int)(__fns(fm, 0, j + 1) & 31u) : lane - sub;          // owner's first lane
+      const int retl = ksh ? __popc(fm & ((1u << (lane - sub)) - 1u)) << lsh : lane;  // where my cell's sums end up
+      const long long cellB = __shfl_sync(FULL, cell, own);
+      const bool t0 = __shfl_sync(FULL, trips, own) == 0;   // first trip: F_g^(t) is still in the state, save it to the scratch
+      const double chisB = __shfl_sync(FULL, chis, own);
+      const double v0 = __shfl_sync(FULL, momk0 * inv_rho, own), v1 = __shfl_sync(FULL, momk1 * inv_rho, own),
+                   v2 = __shfl_sync(FULL, momk2 * inv_rho, own);
+      // sum over the LB lanes of a block, handed to the lanes of the owning cell
+      auto pass_sum = [&](double v) {
+#pragma unroll
+        for (int off = 1; off < 32; off <<= 1)
+          if (off < L || off < LB) v += __shfl_xor_sync(FULL, v, off);
+        return __shfl_sync(FULL, v, retl);
+      };
       double sumR = 0.0, sumAbsR = 0.0, dF0 = 0.0, dF1 = 0.0, dF2 = 0.0;
       int rel_bad = 0;
       char* const pE = reinterpret_cast<char*>(S.Erad);
       char* const pF0 = reinterpret_cast<char*>(S.Frad[0]);
       char* const pF1 = reinterpret_cast<char*>(S.Frad[1]);
       char* const pF2 = reinterpret_cast<char*>(S.Frad[2]);
-      const long long dstep = (long long)L * stride * 8;
-      long long oc = ((long long)sub * stride + cell) * 8, oc_cur = oc;      // group g = i*L + sub
+      // group g = i*LB + subB of the owner sits at step g/L of its lane g%L
+      const int NGB = (Nq + LB - 1) >> lsh;
+      const int col = own + (subB & (L - 1)) - lane;                 // owner's column relative to mine
+      constexpr int SS = NQL * THREADS;                              // slot stride in shared memory
+      double* const sp0 = smem + (subB >> LOG2L) * THREADS + tid + col;
+      double* sp = sp0;
+      const int sst = THREADS << ksh;
+      const long long dstep = ((long long)stride << lsh) * 8, fst = tthreads << ksh;
+      long long oc = ((long long)subB * stride + cellB) * 8, oc_cur = oc;
       auto ldd = [](const char* p, long long o) { return *reinterpret_cast<const double*>(p + o); };
-      double* ftp = scratch + gtid;                    // F_g^(t) scratch of this lane: step i at ftp, components ftc apart
+      double* ftp = scratch + (long long)(subB >> LOG2L) * tthreads + gtid + col;   // F_g^(t): components ftc apart
       const long long ftc = (long long)NQL * tthreads;
       double nEt = 0.0, nFt0 = 0.0, nFt1 = 0.0, nFt2 = 0.0, nFk0 = 0.0, nFk1 = 0.0, nFk2 = 0.0;
-      if (fx && sub < Nq) {
+      if (fx && subB < Nq) {
         nEt = ldd(pE, oc);
         nFk0 = ldd(pF0, oc); nFk1 = ldd(pF1, oc); nFk2 = ldd(pF2, oc);
         if (!t0) { nFt0 = ftp[0]; nFt1 = ftp[ftc]; nFt2 = ftp[2 * ftc]; }
       }
 #pragma unroll 1
-      for (int i = 0; i < NG; ++i) {       // executed by all lanes with per-lane predicates, like loop A
-        const int g = i * L + sub;
+      for (int i = 0; i < NGB; ++i) {      // executed by all lanes with per-lane predicates, like loop A
+        const int g = (i << lsh) + subB;
         const bool vg = fx && g < Nq;
         const int gi = g < Nq ? g : 0;
         const double Et = nEt, Fk0 = nFk0, Fk1 = nFk1, Fk2 = nFk2;
         const double Ft0 = t0 ? nFk0 : nFt0, Ft1 = t0 ? nFk1 : nFt1, Ft2 = t0 ? nFk2 : nFt2;
         oc_cur = oc;
         oc += dstep;
-        if (fx && g + L < Nq) {
+        if (fx && g + LB < Nq) {
           nEt = ldd(pE, oc);
           nFk0 = ldd(pF0, oc); nFk1 = ldd(pF1, oc); nFk2 = ldd(pF2, oc);
-          if (!t0) { nFt0 = ftp[tthreads]; nFt1 = ftp[tthreads + ftc]; nFt2 = ftp[tthreads + 2 * ftc]; }
+          if (!t0) { nFt0 = ftp[fst]; nFt1 = ftp[fst + ftc]; nFt2 = ftp[fst + 2 * ftc]; }
         }
-        const double R = smG(SL_R, i);
+        // (a lane beyond the last group would read past its owner's column: g/L may exceed NQL-1)
+        const double R = g < Nq ? sp[SL_R * SS] : 0.0;
         const double Enew = Et + R;                               // E_g^(t+1) = E_g^(t) + R_g
         double p0, p1, p2;
         closure_vP(P.closure, Enew, Fk0, Fk1, Fk2, v0, v1, v2, c, p0, p1, p2);
-        const double w = s_tab[(gi + 1) * TS + 6] * (chis * s_tab[(gi + 1) * TS + 3]);   // (1 + alpha) chi_E
-        const double chiF = smG(SL_CHIF, i), A = smG(SL_AG, i);
+        const double w = s_tab[(gi + 1) * TS + 6] * (chisB * s_tab[(gi + 1) * TS + 3]);   // (1 + alpha) chi_E
+        const double chiF = g < Nq ? sp[SL_CHIF * SS] : 0.0, A = g < Nq ? sp[SL_AG * SS] : 0.0;
         const double dn = fma(cdt, chiF, 1.0);                    // 1 + c_hat chi_F dt > 0 (guarded in A)
         const bool dn_ok = dn > 1e-290 && dn < 1e290;
         double inv_dn = fast_rcp(dn_ok ? dn : 1.0);
@@ -469,35 +503,39 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
           *reinterpret_cast<double*>(pF0 + oc_cur) = Fn0;
           *reinterpret_cast<double*>(pF1 + oc_cur) = Fn1;
           *reinterpret_cast<double*>(pF2 + oc_cur) = Fn2;
-          smG(SL_DA, i) = Fn0; smG(SL_DB, i) = Fn1; smG(SL_AG, i) = Fn2;   // kept on chip for loop C
+          sp[SL_DA * SS] = Fn0; sp[SL_DB * SS] = Fn1; sp[SL_AG * SS] = Fn2;   // kept on chip for loop C
         }
-        ftp += tthreads;
+        ftp += fst;
+        sp += sst;
       }
-      sumR = cell_sum<L>(sumR); sumAbsR = cell_sum<L>(sumAbsR);
-      dF0 = cell_sum<L>(dF0); dF1 = cell_sum<L>(dF1); dF2 = cell_sum<L>(dF2);
+      sumR = pass_sum(sumR); sumAbsR = pass_sum(sumAbsR);
+      dF0 = pass_sum(dF0); dF1 = pass_sum(dF1); dF2 = pass_sum(dF2);
       double momn0 = 0.0, momn1 = 0.0, momn2 = 0.0, dW = 0.0;
-      if (fx) {
+      if (fxo) {
         momn0 = momt0 - dF0 * icc; momn1 = momt1 - dF1 * icc; momn2 = momt2 - dF2 * icc;   // Eq. 52
         trips++;
         if (COUNT && sub == 0) flops += kFlopOuterCell + kFlopOuterGroup * Nq;
       }
-      const double vn0 = momn0 * inv_rho, vn1 = momn1 * inv_rho, vn2 = momn2 * inv_rho;
+      const double vn0 = __shfl_sync(FULL, momn0 * inv_rho, own), vn1 = __shfl_sync(FULL, momn1 * inv_rho, own),
+                   vn2 = __shfl_sync(FULL, momn2 * inv_rho, own);
+      sp = sp0;
 #pragma unroll 1
-      for (int i = 0; i < NG; ++i) {
-        const int g = i * L + sub;
+      for (int i = 0; i < NGB; ++i) {
+        const int g = (i << lsh) + subB;
         if (fx && g < Nq) {
-          const double vFn = fma(vn0, smG(SL_DA, i), fma(vn1, smG(SL_DB, i), vn2 * smG(SL_AG, i)));
-          const double wf = s_tab[(g + 1) * TS + 6] * smG(SL_CHIF, i) * inv_c;
-          dW += fabs(wf * (vFn - smG(SL_VF, i)));
-          smG(SL_VF, i) = vFn;                                       // lagged v.F_g of the next trip
+          const double vFn = fma(vn0, sp[SL_DA * SS], fma(vn1, sp[SL_DB * SS], vn2 * sp[SL_AG * SS]));
+          const double wf = s_tab[(g + 1) * TS + 6] * sp[SL_CHIF * SS] * inv_c;
+          dW += fabs(wf * (vFn - sp[SL_VF * SS]));
+          sp[SL_VF * SS] = vFn;                                      // lagged v.F_g of the next trip
         }
+        sp += sst;
       }
-      dW = cell_sum<L>(dW);
-      if (L > 1) {
+      dW = pass_sum(dW);
 #pragma unroll
-        for (int off = 1; off < L; off <<= 1) rel_bad |= __shfl_xor_sync(FULL, rel_bad, off);
-      }
-      if (fx) {
+      for (int off = 1; off < 32; off <<= 1)
+        if (off < L || off < LB) rel_bad |= __shfl_xor_sync(FULL, rel_bad, off);
+      rel_bad = __shfl_sync(FULL, rel_bad, retl);
+      if (fxo) {
         bool rel_ok = rel_bad == 0;
         const double Egas_new = Egas_t - c_over_chat * sumR;
         if (P.outer_stop == 1) {
