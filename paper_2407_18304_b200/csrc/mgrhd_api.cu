@@ -181,10 +181,10 @@ struct Inst {
 #define MGRHD_DISPATCH(Nq, WHAT)                               \
   do {                                                         \
     if ((Nq) <= 4) { WHAT(1, 5, 256); }                        \
-    else if ((Nq) <= 8) { WHAT(1, 9, 256); }                   \
+    else if ((Nq) <= 8) { WHAT(1, 9, 384); }                   \
     else if ((Nq) <= 16) { WHAT(2, 9, 384); }                  \
     else if ((Nq) <= 32) { WHAT(4, 9, 384); }                  \
-    else { WHAT(8, 9, 384); }                                  \
+    else { WHAT(4, 17, 256); }                                 \
   } while (0)
 
 // Fills ctx->cfg_* for ctx->P.Nq (called once by mgrhd_init).
