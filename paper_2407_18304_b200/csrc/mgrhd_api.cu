@@ -157,7 +157,7 @@ struct mgrhd_ctx {
 // with as many threads per SM as the register file allows.
 template <int L, int NQL, int THREADS>
 struct Inst {
-  static constexpr size_t kSmem = ((size_t)SL_COUNT * NQL + 1) * THREADS * sizeof(double);   // + one padding row
+  static constexpr size_t kSmem = (size_t)SL_COUNT * NQL * THREADS * sizeof(double);
   static cudaError_t configure(int* blocks_per_sm) {
     cudaError_t e = cudaFuncSetAttribute(source_update_kernel<L, NQL, THREADS, false>,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem);
@@ -176,15 +176,15 @@ struct Inst {
   }
 };
 
-// WHAT(L, NQL, THREADS): lanes per cell, steps per lane (L*NQL >= Nq+1), CTA size -- measured best
+// WHAT(L, NQL, THREADS): lanes per cell, steps per lane (L*NQL >= Nq), CTA size -- measured best
 // on B200 for each bracket of Nq.
 #define MGRHD_DISPATCH(Nq, WHAT)                               \
   do {                                                         \
-    if ((Nq) <= 4) { WHAT(1, 5, 256); }                        \
-    else if ((Nq) <= 8) { WHAT(1, 9, 384); }                   \
-    else if ((Nq) <= 16) { WHAT(2, 9, 384); }                  \
-    else if ((Nq) <= 32) { WHAT(4, 9, 384); }                  \
-    else { WHAT(4, 17, 256); }                                 \
+    if ((Nq) <= 4) { WHAT(1, 4, 256); }                        \
+    else if ((Nq) <= 8) { WHAT(1, 8, 384); }                   \
+    else if ((Nq) <= 16) { WHAT(2, 8, 384); }                  \
+    else if ((Nq) <= 32) { WHAT(4, 8, 384); }                  \
+    else { WHAT(4, 16, 256); }                                 \
   } while (0)
 
 // Fills ctx->cfg_* for ctx->P.Nq (called once by mgrhd_init).

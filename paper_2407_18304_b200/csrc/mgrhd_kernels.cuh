@@ -94,14 +94,15 @@ __device__ __forceinline__ double cell_sum(double v) {
   return v;
 }
 
-// L: lanes that share one cell (1, 2, 4 or 8); lane `sub` of a cell owns edges e = i*L + sub and
-//    the groups g = e-1 below them, i = 0..NQL-1 ("steps"), so the L lanes of a cell evaluate
-//    NEIGHBOURING edges in the same step (x differs by r_g^(L-1) at most: same branch of
+// L: lanes that share one cell (1, 2, 4 or 8); lane `sub` of a cell owns the groups g = i*L + sub,
+//    i = 0..ceil(Nq/L)-1 ("steps"), and their UPPER edges e = g + 1, so the L lanes of a cell
+//    evaluate NEIGHBOURING edges in the same step (x differs by r_g^(L-1) at most: same branch of
 //    planck_edge almost always) and the lower edge of a group comes from the lane to the left
-//    by one shuffle.  A warp works on 32/L cells at a time; per-thread state shrinks by L, so
-//    L times more threads fit beside the same shared memory.
-// NQL: steps per lane, NQL*L >= Nq+1.   THREADS: CTA size.
-// Dynamic shared memory: (SL_COUNT * NQL + 1) * THREADS doubles: one padding row, then [slot][step][thread].
+//    by one shuffle (for lane 0 from the cell's last lane of the previous step, for group 0 from
+//    the per-evaluation prologue, which evaluates edge 0).  A warp works on 32/L cells at a time;
+//    per-thread state shrinks by L, so L times more threads fit beside the same shared memory.
+// NQL: steps per lane the instantiation has room for, NQL*L >= Nq.   THREADS: CTA size.
+// Dynamic shared memory: SL_COUNT * NQL * THREADS doubles, laid out [slot][step][thread].
 // scratch: 3 * NQL * (gridDim.x*THREADS) doubles of global memory, private to this launch:
 //    F_g^(t) of the cell in flight (the state's Frad holds the lagged F_g,k in place).
 //
@@ -117,8 +118,7 @@ template <int L, int NQL, int THREADS, bool COUNT>
 __global__ void __launch_bounds__(THREADS, 1)
 source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ StatePtrs S,
                      unsigned long long* __restrict__ stats, double* __restrict__ scratch) {
-  extern __shared__ double smem_raw[];
-  double* const smem = smem_raw + THREADS;   // one row of padding: loop A's shifted column of step 0 stays in bounds
+  extern __shared__ double smem[];
   __shared__ unsigned int s_hist[2 * MGRHD_HIST];
   // Per-edge table rows in shared memory, row e = {nu_e, and for the group below edge e: k_lo, k_hi,
   // k_mean, 1/k_mean, (4+alpha) k_mean, 1+alpha, (1+alpha)/k_mean}.  The L lanes of a cell read L neighbouring rows per step
@@ -152,14 +152,12 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
 
   const long long tthreads = (long long)gridDim.x * THREADS;
   const long long gtid = (long long)blockIdx.x * THREADS + tid;
-  // Per-group values live in shared memory in GROUP order: group g at step g/L of lane g%L of its
-  // cell (smG), so the flux loops B and C take ceil(Nq/L) full steps.  Loop A walks EDGES
-  // (e = i*L + sub, group g = e - 1): its group sits one lane to the left, or for sub == 0 in the
-  // previous step of the cell's last lane -- a fixed per-lane offset (smA).
-  const int shiftA = sub ? -1 : (L - 1) - THREADS;
+  // Per-group values live in shared memory as [slot][step][thread]: group g = i*L + sub at step i of
+  // lane sub of its cell, for loop A (whose lane owns the UPPER edge e = g + 1 of its group) and the
+  // flux loops alike.
   auto smG = [&](int s, int i) -> double& { return smem[(s * NQL + i) * THREADS + tid]; };
-  auto sm = [&](int s, int i) -> double& { return smem[(s * NQL + i) * THREADS + tid + shiftA]; };
-  const int NG = (Nq + L - 1) / L;                 // steps of the flux loops
+  auto sm = smG;
+  const int NG = (Nq + L - 1) / L;                 // steps per evaluation and per flux pass (<= NQL)
   // scratch: F_g^(t), component k, step i of this lane at scratch[(k*NQL + i)*tthreads + gtid] (coalesced)
 
   // this warp's contiguous chunk of cells [next, end)
@@ -239,7 +237,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
 
     // ===== A: all edges/groups at the trial temperature (a1-a5), then Eq. 49 =======================
     if (__any_sync(FULL, phase == PH_EVAL)) {
-      __syncwarp();        // loop C's v.F_g (group order) is read through the shifted column
+      __syncwarp();        // loop C's v.F_g may have been written by another lane of the warp
       const bool ev = phase == PH_EVAL;
       const bool fin = fin_cell >= 0;
       const double T = ev ? (Egs - Ekin) * inv_Cv : 1.0;
@@ -254,12 +252,22 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
       const double v0 = momk0 * inv_rho, v1 = momk1 * inv_rho, v2 = momk2 * inv_rho;
       double sumR = 0.0, sumAbsFR = 0.0, SFRq = 0.0, SJq = 0.0, sumEt = 0.0;
       int eflops = 0;
-      double prev_yz = 0.0, prev_xi = 0.0;           // this lane's edge of the previous step
-      int prev_small = 1;
+      // edge 0 of the cell, the lower edge of group 0: evaluated here by every lane of the cell, so that
+      // the Nq upper edges fill ceil(Nq/L) steps exactly (Nq + 1 edges in the loop would cost a whole
+      // extra step for one edge).  It is almost always in the Rayleigh-Jeans branch.
+      double prev_yz, prev_xi;                       // this lane's edge of the previous step
+      int prev_small;
+      {
+        bool sm0;
+        int f0;
+        planck_edge0(ev ? P.nu[0] * beta : __longlong_as_double(0x7ff8000000000000ll), prev_yz, prev_xi, sm0, f0);
+        prev_small = sm0;
+        if (COUNT && sub == 0) eflops += f0;
+      }
       const int src = sub == 0 ? lane + (L - 1) : lane - 1;   // lane that owns the lower edge
       const bool last = sub == L - 1;
       const bool evf = ev && first, evp = ev && pend;
-      // register prefetch of the next step's global operands (group g = e - 1, e = i*L + sub).
+      // register prefetch of the next step's global operands (group g = i*L + sub).
       // Byte offsets of (group, cell) advance by a warp-uniform stride per step, so each stream
       // costs one 64-bit add and one load.
       const char* const pE = reinterpret_cast<const char*>(S.Erad);
@@ -267,12 +275,12 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
       const char* const pF1 = reinterpret_cast<const char*>(S.Frad[1]);
       const char* const pF2 = reinterpret_cast<const char*>(S.Frad[2]);
       const long long dstep = (long long)L * stride * 8;
-      long long oc = ((long long)(sub - 1) * stride + cell) * 8;        // (g, cell) of the step being loaded
-      long long of = ((long long)(sub - 1) * stride + fin_cell) * 8;    // (g, fin_cell)
+      long long oc = ((long long)sub * stride + cell) * 8;        // (g, cell) of the step being loaded
+      long long of = ((long long)sub * stride + fin_cell) * 8;    // (g, fin_cell)
       long long of_cur = of;
       double nEt = 0.0, nF0 = 0.0, nF1 = 0.0, nF2 = 0.0, nEo = 0.0;
       auto ldd = [](const char* p, long long o) { return *reinterpret_cast<const double*>(p + o); };
-      if (sub >= 1 && sub - 1 < Nq) {
+      if (sub < Nq) {
         if (ev) nEt = ldd(pE, oc);
         if (evf) { nF0 = ldd(pF0, oc); nF1 = ldd(pF1, oc); nF2 = ldd(pF2, oc); }
         if (fin) nEo = ldd(pE, of);
@@ -281,16 +289,16 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
       // without a cell or without a group in this step computes on harmless values and stores
       // nothing): no divergent branches, so the compiler needs no reconvergence code.
 #pragma unroll 1
-      for (int i = 0; i < NQL; ++i) {
-        const int e = i * L + sub;                   // edge of this lane in this step
-        const int g = e - 1;                         // group below it
-        const bool vg = g >= 0 && g < Nq;
+      for (int i = 0; i < NG; ++i) {
+        const int g = i * L + sub;                   // group of this lane in this step
+        const int e = g + 1;                         // its upper edge
+        const bool vg = g < Nq;
         const bool evg = ev && vg;
         const double Et = nEt, F0 = nF0, F1 = nF1, F2 = nF2, Eo = nEo;
         of_cur = of;
         oc += dstep;
         of += dstep;
-        if (g + L >= 0 && g + L < Nq) {
+        if (g + L < Nq) {
           if (ev) nEt = ldd(pE, oc);
           if (evf) { nF0 = ldd(pF0, oc); nF1 = ldd(pF1, oc); nF2 = ldd(pF2, oc); }
           if (fin) nEo = ldd(pE, of);
@@ -306,7 +314,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
         double hi_yz, hi_xi;
         bool hi_small;
         int hf;
-        planck_edge_w(ev && e <= Nq ? t_nu * beta : __longlong_as_double(0x7ff8000000000000ll),
+        planck_edge_w(evg ? t_nu * beta : __longlong_as_double(0x7ff8000000000000ll),
                       (i & 1) * P.zero, hi_yz, hi_xi, hi_small, hf);
         if (COUNT) eflops += hf;
         double lo_yz, lo_xi;
@@ -403,7 +411,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
 
     // ===== B, C: energy commit (a6), closure + Eq. 51 (a7), Eq. 52 (a8), outer test (a9) ==========
     if (__any_sync(FULL, phase == PH_FLUX)) {
-      __syncwarp();        // loop A wrote R_g, chi_F, A_g through the shifted column
+      __syncwarp();        // the flux pass may read another lane's columns
       const bool fxo = phase == PH_FLUX;      // this lane's own cell is in the flux phase
       // Lane assignment of this pass.  Only the w cells in the flux phase have work here (a bit more
       // than half of the warp's cells on average), so the groups of each are spread over LB = L*kS

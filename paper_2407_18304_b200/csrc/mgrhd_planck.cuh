@@ -107,4 +107,41 @@ __device__ __forceinline__ void planck_edge_w(double x, int which, double& yz, d
   }
 }
 
+// The same for callers outside a step loop (table copy 0), compiled once and called: keeps a second
+// copy of the three branches out of the hot kernel's instruction stream.
+struct EdgeOut { double yz, xi; int small, flops; };
+__device__ __noinline__ EdgeOut planck_edge_call(double x) {
+  EdgeOut o;
+  bool sm;
+  planck_edge_w(x, 0, o.yz, o.xi, sm, o.flops);
+  o.small = sm;
+  return o;
+}
+
+// Edge functions of a cell's LOWEST edge, for a converged warp: the Rayleigh-Jeans branch inline
+// (x_0 = h nu_0/(k_B T) is below kXS for any group structure that resolves the spectrum), anything
+// else through planck_edge_call.  x = NaN: no edge, (0, 0, large).
+__device__ __forceinline__ void planck_edge0(double x, double& yz, double& xi, bool& small, int& flops) {
+  const PlanckTables& tb = mgrhd_c_planck[0];
+  const bool inS = x < kXS;
+  const double x2 = x * x;
+  double2 cf = ld_pair(tb.sp[kSmallTerms - 1]);
+  double sy = cf.x, sx = cf.y;
+#pragma unroll
+  for (int n = kSmallTerms - 2; n >= 0; --n) {
+    cf = ld_pair(tb.sp[n]);
+    sy = fma(sy, x2, cf.x);
+    sx = fma(sx, x2, cf.y);
+  }
+  const double cx3 = kC15Pi4 * (x2 * x);
+  yz = inS ? cx3 * fma(x2, sy, fma(-0.125, x, 1.0 / 3.0)) : 0.0;
+  xi = inS ? cx3 * fma(x2, sx, fma(-0.5, x, 1.0)) : 0.0;
+  small = inS;
+  flops = inS ? kFlopEdgeSmall : 0;
+  if (__any_sync(0xffffffffu, x >= kXS)) {
+    const EdgeOut o = planck_edge_call(x);
+    if (x >= kXS) { yz = o.yz; xi = o.xi; small = o.small != 0; flops = o.flops; }
+  }
+}
+
 }  // namespace mgrhd
