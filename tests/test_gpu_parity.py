@@ -166,6 +166,28 @@ def test_degenerate_cells(gpu, oracle_lib):
     assert_parity(ref, got, st0, wl5.c, wl5.c_hat, label="Nq=64, c_hat=0.05c")
 
 
+
+@pytest.mark.parametrize("Nq,lo_exp", [(2, -2.0), (3, -2.0), (5, -3.0), (7, 0.5), (13, -3.0), (27, -3.0),
+                                        (31, 0.5), (33, -3.0), (47, -4.0), (63, -4.0), (50, 0.5)])
+def test_ragged_group_counts(gpu, oracle_lib, Nq, lo_exp):
+    """Group counts that are not a multiple of the lanes per cell (ragged last step of loop A and of
+    the flux loops, every kernel instantiation), and group structures whose LOWEST edge is not in the
+    Rayleigh-Jeans range (lo_exp = 0.5: x_0 = 3.2/T, the called edge-function path of the prologue)."""
+    wl = W.workload(4 if Nq <= 32 else 5, ncells=257)
+    wl.Nq = Nq
+    wl.edges = np.logspace(lo_exp, lo_exp + 4.0 + (2.0 if Nq > 8 else 0.0), Nq + 1)
+    wl.kappa_lo = wl.kappa_lo[:Nq].copy()
+    # wide groups (few of them) with rising opacity can make Eq. 27 negative (DESIGN.md S8): keep alpha <= 0 there
+    wl.alpha = wl.alpha[:Nq].copy() if Nq >= 16 else np.minimum(wl.alpha[:Nq], 0.0)
+    st0 = W.to_numpy(wl.make_state())
+    ref, got, gs, os_ = run_both(gpu, oracle_lib, wl, st0, wl.dt)
+    assert_parity(ref, got, st0, wl.c, wl.c_hat, label=f"Nq={Nq}, lowest edge 1e{lo_exp}")
+    rE, rP = conservation_residual(st0, got, wl.c, wl.c_hat)
+    assert rE <= 1e-13 and rP <= 1e-13, (rE, rP)
+    for key in ("n_newton_unconverged", "n_outer_unconverged", "n_denominator_nonpositive", "n_chiF_guard"):
+        assert gs[key] == os_[key], (key, gs[key], os_[key])
+
+
 def test_invalid_state_left_untouched(gpu, oracle_lib):
     """A cell whose kinetic energy exceeds its total gas energy (T <= 0) is counted and left as is."""
     wl = W.workload(2, ncells=64)
