@@ -1,20 +1,21 @@
 // mgrhd_kernels.cuh -- the per-cell implicit source update (Eq. 37-52)
-// as one persistent CUDA kernel: one THREAD owns one cell from load to store.
+// as one persistent CUDA kernel: L neighbouring lanes own one cell from load to store.
 //
 // Mapping:
-//  * thread-per-cell, because the dominant cost is the Planck edge functions at the Nq+1
-//    group edges, re-evaluated at every trial temperature: with one cell per thread the EDGE
-//    index is warp-uniform, so 32 lanes evaluate the same edge at 32 temperatures and almost
-//    always take the same branch of planck_edge(); with lanes mapped to groups every warp
-//    would execute every branch.
-//  * per-(cell,group) iteration state lives in SHARED memory, laid out [slot][group][thread]
-//    (conflict-free 8-byte lanes); the lagged fluxes F_g,k live in a small per-thread global
-//    scratch that stays L2-resident.  Nothing is spilled to local memory.
-//  * the Newton loop inside the outer loop is FLATTENED into one loop whose body is
-//    "evaluate all groups at the trial T", followed by a cheap Newton step or by the
-//    flux/momentum update; a lane whose cell has converged stores it and takes the next cell
-//    of its warp's contiguous chunk at once (no atomics), so unequal iteration counts do not
-//    leave lanes idle: every live lane does one full-width evaluation per loop trip.
+//  * the dominant cost is the Planck edge functions at the Nq+1 group edges, re-evaluated at
+//    every trial temperature, so the unit of SIMT work is one (cell, edge): the L lanes of a cell
+//    evaluate L neighbouring edges per step, a warp 32/L cells at a time, and the three branches
+//    of the edge functions are taken warp-wide.  With a whole warp per cell (lanes = groups)
+//    every warp would execute every branch every time.
+//  * per-(cell,group) iteration state lives in SHARED memory, laid out [slot][step][thread]
+//    (conflict-free 8-byte lanes); the lagged fluxes F_g,k stay in place in the state and
+//    F_g^(t) in a small per-thread global scratch that stays L2-resident.  Nothing is spilled
+//    to local memory.
+//  * the Newton loop inside the outer loop is FLATTENED into one loop per warp whose trip is
+//    "evaluate all groups at the trial T" (loop A), followed by a cheap Newton step or by the
+//    flux/momentum update (loops B, C, spread over the whole warp when few cells need them); a
+//    cell that is finished is replaced by the next cell of the warp's contiguous chunk at once
+//    (no atomics), so unequal iteration counts leave no cell slot idle.
 //
 // Product code; shares nothing with oracle/.
 #pragma once
