@@ -11,7 +11,7 @@ from parity_util import assert_parity, conservation_residual, oracle_model
 
 pytestmark = pytest.mark.gpu
 
-# cells: not a multiple of the 128-thread CTA nor of 32, spans many CTAs
+# cells: not a multiple of the cells per CTA (96-384) nor of 32, spans many CTAs
 SIZES = {1: 4096, 2: 5000 + 37, 3: 3000 + 19, 4: 2000 + 5, 5: 1000 + 3}
 
 
