@@ -197,9 +197,9 @@ static cudaError_t configure_ctx(mgrhd_ctx* ctx) {
   return e;
 }
 
-// Bytes of lagged-flux scratch one launch needs at most: 3 * NQ doubles per resident thread.
+// Bytes of scratch one launch needs at most: the head (work counter) and 3 * NQL doubles per resident thread.
 static size_t scratch_bytes(const mgrhd_ctx* ctx) {
-  return (size_t)3 * ctx->cfg_nq * sizeof(double) * (size_t)ctx->sm_count * ctx->cfg_bps * ctx->cfg_threads;
+  return kScratchHead * sizeof(double) + (size_t)3 * ctx->cfg_nq * sizeof(double) * (size_t)ctx->sm_count * ctx->cfg_bps * ctx->cfg_threads;
 }
 
 extern "C" {
@@ -292,6 +292,7 @@ static int launch_update(mgrhd_ctx* ctx, const StatePtrs& S, long long n, long l
   const long long want = (n + cells_per_cta - 1) / cells_per_cta;
   if (blocks > want) blocks = want;
   const bool count = ctx->count_flops != 0;
+  CU(cudaMemsetAsync(scratch, 0, kScratchHead * sizeof(double), st));   // work counter of the chunk scheduler
 #define MGRHD_GO(LL, Q, T) Inst<LL, Q, T>::launch(count, (unsigned)blocks, st, P, S, ctx->d_stats, scratch)
   MGRHD_DISPATCH(P.Nq, MGRHD_GO);
 #undef MGRHD_GO

@@ -83,6 +83,8 @@ __device__ __forceinline__ void closure_vP(int closure, double E, double F0, dou
 // Lane phases of the flattened iteration.
 enum Phase : int { PH_LOAD = 0, PH_EVAL = 1, PH_FLUX = 2, PH_DONE = 3 };
 
+constexpr int kScratchHead = 32;   // doubles in front of the F^(t) scratch (work counter)
+
 // Per-lane, per-local-group shared-memory slots.  DA/DB/AG are reused for F_g^(new) between the
 // two flux passes.
 enum Slot : int { SL_R = 0, SL_DA, SL_DB, SL_VF, SL_AG, SL_CHIF, SL_COUNT };
@@ -104,11 +106,13 @@ __device__ __forceinline__ double cell_sum(double v) {
 //    per-thread state shrinks by L, so L times more threads fit beside the same shared memory.
 // NQL: steps per lane the instantiation has room for, NQL*L >= Nq.   THREADS: CTA size.
 // Dynamic shared memory: SL_COUNT * NQL * THREADS doubles, laid out [slot][step][thread].
-// scratch: 3 * NQL * (gridDim.x*THREADS) doubles of global memory, private to this launch:
-//    F_g^(t) of the cell in flight (the state's Frad holds the lagged F_g,k in place).
+// scratch0: global memory private to this launch: kScratchHead doubles whose first 8 bytes are the
+//    work counter (zero at launch), then 3 * NQL * (gridDim.x*THREADS) doubles: F_g^(t) of the
+//    cell in flight (the state's Frad holds the lagged F_g,k in place).
 //
 // One trip of the main loop, per warp (all loops over steps are entered warp-wide):
-//   LOAD  cells-slots without a cell take the next cells of the warp's chunk (scalars only);
+//   LOAD  cells-slots without a cell take the next cells of the warp's chunk, the warp a new chunk
+//         when it runs out (scalars only);
 //   A     every lane with a cell evaluates its edges/groups at the trial T (a1-a5); the Newton
 //         update of R_g decided in the previous trip is applied on the fly, the first evaluation
 //         of a cell also forms v.F_g and sum E_g, and a lane that has just finished a cell
@@ -118,9 +122,12 @@ __device__ __forceinline__ double cell_sum(double v) {
 template <int L, int NQL, int THREADS, bool COUNT>
 __global__ void __launch_bounds__(THREADS, 1)
 source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ StatePtrs S,
-                     unsigned long long* __restrict__ stats, double* __restrict__ scratch) {
+                     unsigned long long* __restrict__ stats, double* __restrict__ scratch0) {
+  unsigned long long* const work = reinterpret_cast<unsigned long long*>(scratch0);   // next cell to hand out
+  double* const scratch = scratch0 + kScratchHead;
   extern __shared__ double smem[];
   __shared__ unsigned int s_hist[2 * MGRHD_HIST];
+  __shared__ unsigned int s_cnt[8];   // per-CTA counters of rare events, indexed by StatSlot (registers are scarce)
   // Per-edge table rows in shared memory, row e = {nu_e, and for the group below edge e: k_lo, k_hi,
   // k_mean, 1/k_mean, (4+alpha) k_mean, 1+alpha, (1+alpha)/k_mean}.  The L lanes of a cell read L neighbouring rows per step
   // (broadcast within equal `sub`), which would otherwise be lane-indexed constant loads that miss
@@ -128,6 +135,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
   constexpr int TS = 10;   // row stride in doubles: 80 B puts the L rows of a step on distinct banks
   __shared__ __align__(16) double s_tab[(kMaxG + 1) * TS];
   for (int t = threadIdx.x; t < 2 * MGRHD_HIST; t += THREADS) s_hist[t] = 0u;
+  if (threadIdx.x < 8) s_cnt[threadIdx.x] = 0u;
   for (int r = threadIdx.x; r <= P.Nq; r += THREADS) {
     const int g = r > 0 ? r - 1 : 0;
     s_tab[r * TS + 0] = P.nu[r];
@@ -161,15 +169,26 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
   const int NG = (Nq + L - 1) / L;                 // steps per evaluation and per flux pass (<= NQL)
   // scratch: F_g^(t), component k, step i of this lane at scratch[(k*NQL + i)*tthreads + gtid] (coalesced)
 
-  // this warp's contiguous chunk of cells [next, end)
-  const long long nwarps = tthreads >> 5, wid = gtid >> 5;
-  const long long per = (n + nwarps - 1) / nwarps;
-  long long next = wid * per;
-  const long long end = next + per < n ? next + per : n;
-  if (next > n) next = n;
+  // Large problems: cells are handed to the warps in chunks of consecutive cells from a counter in
+  // global memory (zeroed by the host before the launch), because the SMs do not all run at the
+  // same rate (with equal shares the slowest took 13 % longer than the fastest: -4 % at 256^3 cells).
+  // A chunk is 1/64 of a warp's fair share (the warps finish within one chunk of one another), at
+  // most 128 cells (1 KB of every array).  Below 1024 cells per warp the bookkeeping costs more than
+  // the balance gains and every warp takes one contiguous share.  Either way a cell's result does
+  // not depend on the warp that computes it.
+  const long long nwarps = tthreads >> 5;
+  long long next = 0, end = 0;      // the warp's current chunk [next, end)
+  bool exhausted = false;           // no further chunk to take
+  if (n < nwarps * 1024) {
+    const long long per = (n + nwarps - 1) / nwarps;
+    next = (gtid >> 5) * per;
+    end = next + per < n ? next + per : n;
+    if (next > n) next = n;
+    exhausted = true;
+  }
 
-  unsigned int cnt_newton_unconv = 0, cnt_outer_unconv = 0, cnt_Tnonpos = 0, cnt_guard = 0,
-               cnt_den = 0, cnt_evals = 0, cnt_trips = 0, cnt_cells = 0;
+  // (failures are rare: they go straight to the global counters; cells are counted from the histogram)
+  unsigned int cnt_guard = 0, cnt_den = 0, cnt_evals = 0, cnt_trips = 0;
   unsigned long long flops = 0;
 
   // ---- per-cell state, replicated in the L lanes of the cell ------------------------------------
@@ -193,7 +212,6 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
     if (sub == 0) {
       cnt_evals += evals;
       cnt_trips += trips;
-      cnt_cells++;
       atomicAdd(&s_hist[evals < MGRHD_HIST ? evals : MGRHD_HIST - 1], 1u);
       atomicAdd(&s_hist[MGRHD_HIST + (trips < MGRHD_HIST ? trips : MGRHD_HIST - 1)], 1u);
     }
@@ -202,37 +220,53 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
 
   while (true) {
     // ===== LOAD (a0): scalars of the next cell of the warp's chunk ================================
-    const unsigned need = __ballot_sync(FULL, phase == PH_LOAD) & LEADERS;
-    if (need) {
-      if (phase == PH_LOAD) {
-        const long long cnew = next + __popc(need & ((1u << (lane - sub)) - 1u));
-        if (cnew < end) {
-          cell = cnew;
-          rho = S.rho[cell];
-          const double ks = S.kappa_scale ? S.kappa_scale[cell] : 1.0;
-          momt0 = S.mom[0][cell]; momt1 = S.mom[1][cell]; momt2 = S.mom[2][cell];
-          Egas_t = S.Egas[cell];
-          chis = rho * ks;                      // chi_{g-} = chis * k_lo[g]
-          inv_chis = 1.0 / chis;
-          inv_rho = 1.0 / rho;
-          inv_Cv = 1.0 / (rho * P.cv_over_rho);
-          momk0 = momt0; momk1 = momt1; momk2 = momt2;
-          Egs = Egas_t;
-          Ekin = (momk0 * momk0 + momk1 * momk1 + momk2 * momk2) * (0.5 * inv_rho);
-          it = 0; k = 0; evals = 0; trips = 0;
-          first = true; pend = false;
-          if (COUNT && sub == 0) flops += kFlopCell + kFlopCellGroup * Nq;
-          if ((Egs - Ekin) * inv_Cv > 0.0) {
-            phase = PH_EVAL;
-          } else {                              // invalid state: count it, leave the cell as it is
-            if (sub == 0) cnt_Tnonpos++;
-            finish(0.0, 0.0, 0.0, 0.0);
-          }
-        } else {
-          phase = PH_DONE;
+    unsigned need = __ballot_sync(FULL, phase == PH_LOAD) & LEADERS;   // cell slots to fill (first lanes)
+    while (need) {                                                      // warp-uniform
+      if (next >= end) {                                                // next chunk
+        if (exhausted) {
+          if (phase == PH_LOAD) phase = PH_DONE;
+          break;
+        }
+        long long CH = n / (nwarps * 64);
+        CH = CH > 128 ? 128 : CH;
+        unsigned long long b = 0;
+        if (lane == 0) b = atomicAdd(work, (unsigned long long)CH);
+        b = __shfl_sync(FULL, b, 0);
+        if ((long long)b >= n) { exhausted = true; continue; }
+        next = (long long)b;
+        end = next + CH < n ? next + CH : n;
+      }
+      // hand the cells next, next + 1, ... of the chunk to the slots in `need`, lowest lanes first
+      const long long avail = end - next;
+      const int r = __popc(need & ((1u << (lane - sub)) - 1u));        // my slot's place among them
+      const bool mine = ((need >> (lane - sub)) & 1u) != 0;
+      if (phase == PH_LOAD && mine && r < avail) {
+        cell = next + r;
+        rho = S.rho[cell];
+        const double ks = S.kappa_scale ? S.kappa_scale[cell] : 1.0;
+        momt0 = S.mom[0][cell]; momt1 = S.mom[1][cell]; momt2 = S.mom[2][cell];
+        Egas_t = S.Egas[cell];
+        chis = rho * ks;                      // chi_{g-} = chis * k_lo[g]
+        inv_chis = 1.0 / chis;
+        inv_rho = 1.0 / rho;
+        inv_Cv = 1.0 / (rho * P.cv_over_rho);
+        momk0 = momt0; momk1 = momt1; momk2 = momt2;
+        Egs = Egas_t;
+        Ekin = (momk0 * momk0 + momk1 * momk1 + momk2 * momk2) * (0.5 * inv_rho);
+        it = 0; k = 0; evals = 0; trips = 0;
+        first = true; pend = false;
+        if (COUNT && sub == 0) flops += kFlopCell + kFlopCellGroup * Nq;
+        if ((Egs - Ekin) * inv_Cv > 0.0) {
+          phase = PH_EVAL;
+        } else {                              // invalid state: count it, leave the cell as it is
+          if (sub == 0) atomicAdd(&stats[kStatTNonPos], 1ull);
+          finish(0.0, 0.0, 0.0, 0.0);         // (its slot is refilled in the next trip)
         }
       }
-      next += __popc(need);
+      const int wanted = __popc(need);
+      const int given = wanted < avail ? wanted : (int)avail;
+      next += given;
+      need = __ballot_sync(FULL, mine && sub == 0 && r >= given);      // slots the chunk had no cell for
     }
     if (__all_sync(FULL, phase == PH_DONE)) break;
 
@@ -390,7 +424,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
         if (conv) {
           phase = PH_FLUX;                                          // Eq. 49 met
         } else if (it >= P.newton_maxit) {
-          if (sub == 0) cnt_newton_unconv++;
+          if (sub == 0) atomicAdd(&stats[kStatNewtonUnconv], 1ull);
           phase = PH_FLUX;
         } else {
           // Newton step: eliminate the gas row
@@ -399,7 +433,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
           lam = 1.0;
           for (int h = 0; h < 10 && !((Egs + lam * dx0 - Ekin) * inv_Cv > 0.0); ++h) {
             lam *= 0.5;
-            if (sub == 0) cnt_Tnonpos++;
+            if (sub == 0) atomicAdd(&stats[kStatTNonPos], 1ull);
           }
           Egs += lam * dx0;
           ldx = lam * dx0;
@@ -415,16 +449,18 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
       __syncwarp();        // the flux pass may read another lane's columns
       const bool fxo = phase == PH_FLUX;      // this lane's own cell is in the flux phase
       // Lane assignment of this pass.  Only the w cells in the flux phase have work here (a bit more
-      // than half of the warp's cells on average), so the groups of each are spread over LB = L*kS
-      // lanes, kS the largest power of two with w*LB <= 32: block j of LB lanes works for the j-th
-      // flux cell ("owner"), reads its scalars by shuffle and its per-group columns in shared memory
-      // and in the scratch directly, and hands the sums back.  kS = 1 is the plain case: every lane
-      // works for its own cell.
+      // than half of the warp's cells on average): when they are at most half, the groups of each are
+      // spread over LB = 2L lanes -- block j of 2L lanes works for the j-th flux cell ("owner"), reads
+      // its scalars by shuffle and its per-group columns in shared memory and in the scratch directly,
+      // and hands the sums back.  Lane s of a cell then does the even steps of column s and lane s + L
+      // the odd ones; the plain pass (LB = L, every lane works for its own cell) keeps separate sums
+      // over even and odd steps, so both form every sum in the same order and a cell's result does
+      // not depend on which other cells of its warp were in the flux phase (bit-reproducible
+      // whatever the scheduling).
       constexpr int LOG2L = L == 1 ? 0 : (L == 2 ? 1 : (L == 4 ? 2 : 3));
       const unsigned fm = __ballot_sync(FULL, fxo) & LEADERS;
       const int w = __popc(fm);
-      int ksh = 0;
-      while (((w * L) << (ksh + 1)) <= 32) ++ksh;
+      const int ksh = 2 * w * L <= 32 ? 1 : 0;
       const int lsh = ksh + LOG2L, LB = 1 << lsh;
       const int subB = lane & (LB - 1), j = lane >> lsh;
       const bool fx = ksh ? j < w : fxo;
@@ -435,15 +471,16 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
       const double chisB = __shfl_sync(FULL, chis, own);
       const double v0 = __shfl_sync(FULL, momk0 * inv_rho, own), v1 = __shfl_sync(FULL, momk1 * inv_rho, own),
                    v2 = __shfl_sync(FULL, momk2 * inv_rho, own);
-      // sum over the LB lanes of a block, handed to the lanes of the owning cell
-      auto pass_sum = [&](double v) {
+      double sumR = 0.0, sumAbsR = 0.0, dF0 = 0.0, dF1 = 0.0, dF2 = 0.0;        // even steps (all steps of a 2L-lane worker)
+      double sumRo = 0.0, sumAbsRo = 0.0, dF0o = 0.0, dF1o = 0.0, dF2o = 0.0;   // odd steps of the plain pass
+      int rel_bad = 0;
+      // (even + odd) of a column, then across the L columns of the cell; for 2L lanes the odd half sits L lanes up
+      auto pass_sum = [&](double ve, double vo) {
+        double v = ksh ? ve + __shfl_xor_sync(FULL, ve, L) : ve + vo;
 #pragma unroll
-        for (int off = 1; off < 32; off <<= 1)
-          if (off < L || off < LB) v += __shfl_xor_sync(FULL, v, off);
+        for (int off = 1; off < L; off <<= 1) v += __shfl_xor_sync(FULL, v, off);
         return __shfl_sync(FULL, v, retl);
       };
-      double sumR = 0.0, sumAbsR = 0.0, dF0 = 0.0, dF1 = 0.0, dF2 = 0.0;
-      int rel_bad = 0;
       char* const pE = reinterpret_cast<char*>(S.Erad);
       char* const pF0 = reinterpret_cast<char*>(S.Frad[0]);
       char* const pF1 = reinterpret_cast<char*>(S.Frad[1]);
@@ -502,10 +539,11 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
         bool ok = d2 <= rel2 * f2;
         if (__any_sync(FULL, vg && !sq_ok))
           ok = sq_ok ? ok : norm3(e0, e1, e2) <= P.outer_rel_tol * norm3(Fn0, Fn1, Fn2);
+        const bool odd = !ksh && (i & 1);
+        const double q0 = Fn0 - Ft0, q1 = Fn1 - Ft1, q2 = Fn2 - Ft2;
+        if (vg && !odd) { sumR += R; sumAbsR += fabs(R); dF0 += q0; dF1 += q1; dF2 += q2; }
+        if (vg && odd) { sumRo += R; sumAbsRo += fabs(R); dF0o += q0; dF1o += q1; dF2o += q2; }
         if (vg) {
-          sumR += R;
-          sumAbsR += fabs(R);
-          dF0 += Fn0 - Ft0; dF1 += Fn1 - Ft1; dF2 += Fn2 - Ft2;
           if (P.outer_stop == 1 && !ok) rel_bad = 1;
           if (t0) { ftp[0] = Ft0; ftp[ftc] = Ft1; ftp[2 * ftc] = Ft2; }
           // lagged flux of the next trip, in place
@@ -517,9 +555,9 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
         ftp += fst;
         sp += sst;
       }
-      sumR = pass_sum(sumR); sumAbsR = pass_sum(sumAbsR);
-      dF0 = pass_sum(dF0); dF1 = pass_sum(dF1); dF2 = pass_sum(dF2);
-      double momn0 = 0.0, momn1 = 0.0, momn2 = 0.0, dW = 0.0;
+      sumR = pass_sum(sumR, sumRo); sumAbsR = pass_sum(sumAbsR, sumAbsRo);
+      dF0 = pass_sum(dF0, dF0o); dF1 = pass_sum(dF1, dF1o); dF2 = pass_sum(dF2, dF2o);
+      double momn0 = 0.0, momn1 = 0.0, momn2 = 0.0, dW = 0.0, dWo = 0.0;
       if (fxo) {
         momn0 = momt0 - dF0 * icc; momn1 = momt1 - dF1 * icc; momn2 = momt2 - dF2 * icc;   // Eq. 52
         trips++;
@@ -534,12 +572,13 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
         if (fx && g < Nq) {
           const double vFn = fma(vn0, sp[SL_DA * SS], fma(vn1, sp[SL_DB * SS], vn2 * sp[SL_AG * SS]));
           const double wf = s_tab[(g + 1) * TS + 6] * sp[SL_CHIF * SS] * inv_c;
-          dW += fabs(wf * (vFn - sp[SL_VF * SS]));
+          const double dWg = fabs(wf * (vFn - sp[SL_VF * SS]));
+          if (!ksh && (i & 1)) dWo += dWg; else dW += dWg;
           sp[SL_VF * SS] = vFn;                                      // lagged v.F_g of the next trip
         }
         sp += sst;
       }
-      dW = pass_sum(dW);
+      dW = pass_sum(dW, dWo);
 #pragma unroll
       for (int off = 1; off < 32; off <<= 1)
         if (off < L || off < LB) rel_bad |= __shfl_xor_sync(FULL, rel_bad, off);
@@ -555,7 +594,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
         if (delta <= P.outer_tol * fmax(sumAbsR, Etot) && rel_ok) {
           finish(momn0, momn1, momn2, Egas_new);
         } else if (k == P.outer_maxit - 1) {
-          if (sub == 0) cnt_outer_unconv++;
+          if (sub == 0) atomicAdd(&stats[kStatOuterUnconv], 1ull);
           finish(momn0, momn1, momn2, Egas_new);
         } else {
           momk0 = momn0; momk1 = momn1; momk2 = momn2;
@@ -565,7 +604,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
           if ((Egs - Ekin) * inv_Cv > 0.0) {
             phase = PH_EVAL;
           } else {
-            if (sub == 0) cnt_Tnonpos++;
+            if (sub == 0) atomicAdd(&stats[kStatTNonPos], 1ull);
             finish(momn0, momn1, momn2, Egas_new);
           }
         }
@@ -585,13 +624,13 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
     }
 
   // ---- diagnostics: warp-reduce the scalar counters, one atomic per warp ------------------
-  unsigned int vals[8] = {cnt_cells, cnt_newton_unconv, cnt_outer_unconv, cnt_Tnonpos,
-                          cnt_guard, cnt_den, cnt_evals, cnt_trips};
+  const unsigned int vals[4] = {cnt_guard, cnt_den, cnt_evals, cnt_trips};
+  const int slot[4] = {kStatChiFGuard, kStatDenNonPos, kStatNewtonEvals, kStatOuterTrips};
 #pragma unroll
-  for (int s = 0; s < 8; ++s) {
+  for (int s = 0; s < 4; ++s) {
     unsigned int v = vals[s];
     for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(FULL, v, off);
-    if (lane == 0 && v) atomicAdd(&stats[s], (unsigned long long)v);
+    if (lane == 0 && v) atomicAdd(&stats[slot[s]], (unsigned long long)v);
   }
   if (COUNT) {
     for (int off = 16; off > 0; off >>= 1) flops += __shfl_xor_sync(FULL, flops, off);
@@ -599,7 +638,10 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
   }
   __syncthreads();
   for (int t = threadIdx.x; t < 2 * MGRHD_HIST; t += THREADS)
-    if (s_hist[t]) atomicAdd(&stats[kStatNewtonHist + t], (unsigned long long)s_hist[t]);
+    if (s_hist[t]) {
+      atomicAdd(&stats[kStatNewtonHist + t], (unsigned long long)s_hist[t]);
+      if (t < MGRHD_HIST) atomicAdd(&stats[kStatCells], (unsigned long long)s_hist[t]);   // every finished cell is in one bin
+    }
 }
 
 // Per-cell conserved totals: E_gas + (c/c_hat) sum E_g and

@@ -188,6 +188,41 @@ def test_ragged_group_counts(gpu, oracle_lib, Nq, lo_exp):
         assert gs[key] == os_[key], (key, gs[key], os_[key])
 
 
+
+@pytest.mark.parametrize("index", [2, 3, 4, 5])
+def test_bit_reproducible_and_independent_of_scheduling(gpu, index):
+    """A cell's result depends on that cell alone: the same state updated twice, as a whole or as its
+    first third only (other chunks, other neighbours in the warp, other lane assignments in the flux
+    pass), and through the host-buffer path (slabs), gives the same bits."""
+    import torch
+
+    wl = W.workload(index, ncells=3001)
+    st0 = W.to_numpy(wl.make_state())
+    dt = wl.dt_of_call(0)
+
+    def run(state, host=False):
+        ctx = gpu.Context.from_workload(wl)
+        if host:
+            out = {k: (None if v is None else v.copy()) for k, v in state.items()}
+            ctx.source_update_host(out, dt, wl.c, wl.c_hat)
+        else:
+            dev = {k: (None if v is None else torch.from_numpy(v.copy()).cuda()) for k, v in state.items()}
+            ctx.source_update(dev, dt, wl.c, wl.c_hat)
+            torch.cuda.synchronize()
+            out = W.to_numpy(dev)
+        ctx.free()
+        return out
+
+    a, b, h = run(st0), run(st0), run(st0, host=True)
+    m = 1000
+    part = {k: (None if v is None else np.ascontiguousarray(v[..., :m])) for k, v in st0.items()}
+    c = run(part)
+    for key in ("mom", "Egas", "Erad", "Frad"):
+        assert np.array_equal(a[key], b[key]), key
+        assert np.array_equal(a[key], h[key]), key
+        assert np.array_equal(a[key][..., :m], c[key]), key
+
+
 def test_invalid_state_left_untouched(gpu, oracle_lib):
     """A cell whose kinetic energy exceeds its total gas energy (T <= 0) is counted and left as is."""
     wl = W.workload(2, ncells=64)
