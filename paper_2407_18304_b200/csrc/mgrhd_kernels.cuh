@@ -13,9 +13,12 @@
 //    to local memory.
 //  * the Newton loop inside the outer loop is FLATTENED into one loop per warp whose trip is
 //    "evaluate all groups at the trial T" (loop A), followed by a cheap Newton step or by the
-//    flux/momentum update (loops B, C, spread over the whole warp when few cells need them); a
-//    cell that is finished is replaced by the next cell of the warp's contiguous chunk at once
-//    (no atomics), so unequal iteration counts leave no cell slot idle.
+//    flux/momentum update (loops B, C, over twice the lanes when at most half of the warp's
+//    cells need them); a cell that is finished is replaced at once by the next cell of the warp's
+//    chunk (one atomic per chunk of up to 128 cells, none for small problems), so unequal
+//    iteration counts leave no cell slot idle and unequal SM speeds no SM.
+//  * a cell's result does not depend on the warp, the neighbours or the lane assignment it is
+//    computed with: every sum is formed in one fixed order (bit-reproducible).
 //
 // Product code; shares nothing with oracle/.
 #pragma once
