@@ -175,9 +175,10 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
   // Large problems: cells are handed to the warps in chunks of consecutive cells from a counter in
   // global memory (zeroed by the host before the launch), because the SMs do not all run at the
   // same rate (with equal shares the slowest took 13 % longer than the fastest: -4 % at 256^3 cells).
-  // A chunk is 1/64 of a warp's fair share (the warps finish within one chunk of one another), at
-  // most 128 cells (1 KB of every array).  Below 1024 cells per warp the bookkeeping costs more than
-  // the balance gains and every warp takes one contiguous share.  Either way a cell's result does
+  // A chunk is 64 or 128 cells (whole 128-byte lines of every array: chunks that split lines between
+  // SMs cost more DRAM traffic than the balance gains; at least 16 chunks per warp, so the warps
+  // finish within a few percent of one another).  Below 1024 cells per warp every warp takes one
+  // contiguous share.  Either way a cell's result does
   // not depend on the warp that computes it.
   const long long nwarps = tthreads >> 5;
   long long next = 0, end = 0;      // the warp's current chunk [next, end)
@@ -230,8 +231,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
           if (phase == PH_LOAD) phase = PH_DONE;
           break;
         }
-        long long CH = n / (nwarps * 64);
-        CH = CH > 128 ? 128 : CH;
+        const long long CH = n >= nwarps * 4096 ? 128 : 64;
         unsigned long long b = 0;
         if (lane == 0) b = atomicAdd(work, (unsigned long long)CH);
         b = __shfl_sync(FULL, b, 0);
