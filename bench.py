@@ -329,7 +329,7 @@ def run_ours(args) -> None:
 # `ncu --set full` capture summarised in profiles/r1_final_ncu_full.md: 2.678 + 6.115 GB at
 # 2 097 152 cells of config 4, scaled x8 to its 16 777 216 cells (persistent grid-stride kernel,
 # traffic linear in cells).  None for workloads without a capture.
-NCU_TRAFFIC_BYTES: dict = {4: 8.0 * (2.580806e9 + 5.619502e9)}
+NCU_TRAFFIC_BYTES: dict = {4: 8.0 * (2.895354e9 + 5.651977e9)}
 
 
 def run_e2e(args, wl, ctx, pristine, dt, world, dist):
