@@ -69,3 +69,35 @@ def test_full_size_sampled_parity(oracle_lib, index):
     ctx.free()
     del dev, E0, P0, E1, P1, Es, Ps
     torch.cuda.empty_cache()
+
+
+@pytest.mark.parametrize("index,ncells", [(3, 1 << 21), (4, 1 << 21), (5, 1 << 21)])
+def test_chunked_distribution_is_bit_reproducible(index, ncells):
+    """Sizes at which the warps take chunks from the global counter (who computes which cell then
+    depends on timing): two runs give the same bits, and the first cells the same bits as a small
+    run of those cells alone (one contiguous share per warp, other neighbours, other lane assignments)."""
+    import torch
+
+    if not torch.cuda.is_available():
+        pytest.fail("GPU test selected but no CUDA device is visible")
+    from paper_2407_18304_b200 import binding
+
+    wl = W.workload(index, ncells=ncells)
+    dt = wl.dt_of_call(0)
+    pristine = wl.make_state(device="cuda")
+
+    def run(state):
+        st = {k: (None if v is None else v.clone()) for k, v in state.items()}
+        ctx = binding.Context.from_workload(wl)
+        ctx.source_update(st, dt, wl.c, wl.c_hat)
+        torch.cuda.synchronize()
+        ctx.free()
+        return st
+
+    a, b = run(pristine), run(pristine)
+    m = 3001
+    part = {k: (None if v is None else v[..., :m].contiguous()) for k, v in pristine.items()}
+    c = run(part)
+    for key in ("mom", "Egas", "Erad", "Frad"):
+        assert torch.equal(a[key], b[key]), key
+        assert torch.equal(a[key][..., :m], c[key]), key
