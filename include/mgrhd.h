@@ -100,7 +100,9 @@ int mgrhd_init(mgrhd_ctx **out, const double *group_edges, int Nq,
 /* One implicit source update (Eq. 37-52) of `ncells` cells, in place, with dt = theta*Delta t
  * (PAPER.md:389), speed of light c and reduced speed of light c_hat <= c (Eq. 34).
  * Stream-ordered on `cuda_stream` (a cudaStream_t, NULL = default stream), asynchronous:
- * no host synchronisation, no allocation.  ncells == 0 is a no-op.  Per-cell numerical
+ * no host synchronisation, no allocation (one 256-byte memset of the work counter and one kernel
+ * are enqueued).  ncells == 0 is a no-op.  A cell's result depends on that cell alone: results are
+ * bit-identical from call to call and for any partition of the cells into calls.  Per-cell numerical
  * failures never abort; they are counted in mgrhd_stats.  A context owns one scratch buffer:
  * at most ONE mgrhd_source_update per context may be in flight at a time (calls on the same
  * stream are naturally serialised; use one context per stream for concurrent updates). */
