@@ -467,7 +467,9 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
       const int lsh = ksh + LOG2L, LB = 1 << lsh;
       const int subB = lane & (LB - 1), j = lane >> lsh;
       const bool fx = ksh ? j < w : fxo;
-      const int own = ksh ? (int)(__fns(fm, 0, j + 1) & 31u) : lane - sub;          // owner's first lane
+      // owner's first lane; a block without an owner (j >= w) keeps its own cell's columns, so that its
+      // (unused) reads stay inside the warp's part of shared memory
+      const int own = ksh && fx ? (int)__fns(fm, 0, j + 1) : lane - sub;
       const int retl = ksh ? __popc(fm & ((1u << (lane - sub)) - 1u)) << lsh : lane;  // where my cell's sums end up
       const long long cellB = __shfl_sync(FULL, cell, own);
       const bool t0 = __shfl_sync(FULL, trips, own) == 0;   // first trip: F_g^(t) is still in the state, save it to the scratch
