@@ -1,6 +1,6 @@
 """Build libmgrhd.so (the C-ABI CUDA library) in-tree with nvcc for sm_100a.
 
-    python -m paper_2407_18304_b200.build [--force]
+    python -m paper_2407_18304_b200.build [--force] [--check]
 
 nvcc cross-compiles without a GPU.  The .so is git-ignored but travels to the GPU box.
 """
@@ -39,12 +39,15 @@ def needs_build() -> bool:
     return any(os.path.getmtime(os.path.join(CSRC, d)) > t for d in DEPS)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    if force or needs_build():
-        cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + SOURCES
+def build(force: bool = False, verbose: bool = False, check: bool = False) -> str:
+    """check=True: the bounds-checked debug build (every shared-memory, state and scratch index is
+    tested where it is used; a violation traps).  Always rebuild without it before timing anything."""
+    if force or check or needs_build():
+        cmd = ([_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else [])
+               + (["-DMGRHD_BOUNDS_CHECK"] if check else []) + ["-o", LIB] + SOURCES)
         subprocess.run(cmd, check=True, cwd=CSRC)
     return LIB
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv, check="--check" in sys.argv))

@@ -24,6 +24,22 @@
 #pragma once
 #include "mgrhd_planck.cuh"
 
+// Bounds-checked build (python -m paper_2407_18304_b200.build --check): every index into shared
+// memory, the state and the scratch is tested where it is used, and a violation traps.  This stands
+// in for compute-sanitizer, which this pool does not offer; never on in a timed or released build.
+#ifdef MGRHD_BOUNDS_CHECK
+#define MGRHD_CHK(cond)                                                                       \
+  do {                                                                                        \
+    if (!(cond)) {                                                                            \
+      printf("mgrhd bounds check failed: %s, line %d, block %d thread %d\n", #cond, __LINE__, \
+             (int)blockIdx.x, (int)threadIdx.x);                                              \
+      __trap();                                                                               \
+    }                                                                                         \
+  } while (0)
+#else
+#define MGRHD_CHK(cond) ((void)0)
+#endif
+
 namespace mgrhd {
 
 // ---- fast, IEEE-faithful-to-1-ulp reciprocal / sqrt for NORMAL positive arguments -----------
@@ -167,7 +183,14 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
   // Per-group values live in shared memory as [slot][step][thread]: group g = i*L + sub at step i of
   // lane sub of its cell, for loop A (whose lane owns the UPPER edge e = g + 1 of its group) and the
   // flux loops alike.
-  auto smG = [&](int s, int i) -> double& { return smem[(s * NQL + i) * THREADS + tid]; };
+  auto smG = [&](int s, int i) -> double& {
+    MGRHD_CHK(s >= 0 && s < SL_COUNT && i >= 0 && i < NQL);
+    return smem[(s * NQL + i) * THREADS + tid];
+  };
+  // offsets (in doubles / bytes) inside which every access must stay
+  const long long lim_smem = (long long)SL_COUNT * NQL * THREADS, lim_state = (long long)Nq * stride * 8,
+                  lim_scratch = 3ll * NQL * tthreads;
+  (void)lim_smem; (void)lim_state; (void)lim_scratch;
   auto sm = smG;
   const int NG = (Nq + L - 1) / L;                 // steps per evaluation and per flux pass (<= NQL)
   // scratch: F_g^(t), component k, step i of this lane at scratch[(k*NQL + i)*tthreads + gtid] (coalesced)
@@ -245,6 +268,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
       const bool mine = ((need >> (lane - sub)) & 1u) != 0;
       if (phase == PH_LOAD && mine && r < avail) {
         cell = next + r;
+        MGRHD_CHK(cell >= 0 && cell < n);
         rho = S.rho[cell];
         const double ks = S.kappa_scale ? S.kappa_scale[cell] : 1.0;
         momt0 = S.mom[0][cell]; momt1 = S.mom[1][cell]; momt2 = S.mom[2][cell];
@@ -319,6 +343,8 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
       double nEt = 0.0, nF0 = 0.0, nF1 = 0.0, nF2 = 0.0, nEo = 0.0;
       auto ldd = [](const char* p, long long o) { return *reinterpret_cast<const double*>(p + o); };
       if (sub < Nq) {
+        MGRHD_CHK(!ev || (oc >= 0 && oc < lim_state));
+        MGRHD_CHK(!fin || (of >= 0 && of < lim_state));
         if (ev) nEt = ldd(pE, oc);
         if (evf) { nF0 = ldd(pF0, oc); nF1 = ldd(pF1, oc); nF2 = ldd(pF2, oc); }
         if (fin) nEo = ldd(pE, of);
@@ -337,6 +363,8 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
         oc += dstep;
         of += dstep;
         if (g + L < Nq) {
+          MGRHD_CHK(!ev || (oc >= 0 && oc < lim_state));
+          MGRHD_CHK(!fin || (of >= 0 && of < lim_state));
           if (ev) nEt = ldd(pE, oc);
           if (evf) { nF0 = ldd(pF0, oc); nF1 = ldd(pF1, oc); nF2 = ldd(pF2, oc); }
           if (fin) nEo = ldd(pE, of);
@@ -347,6 +375,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
                      t_wc = r67.y;
         const double Rold = sm(SL_R, i);
         // a10 of the cell this lane finished in the previous trip: E_g^(t+1) = E_g^(t) + R_g
+        MGRHD_CHK(!(fin && vg) || (of_cur >= 0 && of_cur < lim_state));
         if (fin && vg) *reinterpret_cast<double*>(const_cast<char*>(pE) + of_cur) = Eo + Rold;
         // a1: edge functions at this lane's edge; the lower edge of group g comes from the left
         double hi_yz, hi_xi;
@@ -504,6 +533,8 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
       const long long ftc = (long long)NQL * tthreads;
       double nEt = 0.0, nFt0 = 0.0, nFt1 = 0.0, nFt2 = 0.0, nFk0 = 0.0, nFk1 = 0.0, nFk2 = 0.0;
       if (fx && subB < Nq) {
+        MGRHD_CHK(oc >= 0 && oc < lim_state && cellB >= 0 && cellB < n);
+        MGRHD_CHK(t0 || (ftp - scratch >= 0 && ftp - scratch + 2 * ftc < lim_scratch));
         nEt = ldd(pE, oc);
         nFk0 = ldd(pF0, oc); nFk1 = ldd(pF1, oc); nFk2 = ldd(pF2, oc);
         if (!t0) { nFt0 = ftp[0]; nFt1 = ftp[ftc]; nFt2 = ftp[2 * ftc]; }
@@ -518,11 +549,14 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
         oc_cur = oc;
         oc += dstep;
         if (fx && g + LB < Nq) {
+          MGRHD_CHK(oc >= 0 && oc < lim_state);
+          MGRHD_CHK(t0 || (ftp + fst - scratch >= 0 && ftp + fst - scratch + 2 * ftc < lim_scratch));
           nEt = ldd(pE, oc);
           nFk0 = ldd(pF0, oc); nFk1 = ldd(pF1, oc); nFk2 = ldd(pF2, oc);
           if (!t0) { nFt0 = ftp[fst]; nFt1 = ftp[fst + ftc]; nFt2 = ftp[fst + 2 * ftc]; }
         }
         // (a lane beyond the last group would read past its owner's column: g/L may exceed NQL-1)
+        MGRHD_CHK(g >= Nq || (sp - smem >= 0 && sp - smem < SS));      // every slot of this step stays in its slot
         const double R = g < Nq ? sp[SL_R * SS] : 0.0;
         const double Enew = Et + R;                               // E_g^(t+1) = E_g^(t) + R_g
         double p0, p1, p2;
@@ -549,6 +583,8 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
         if (vg && !odd) { sumR += R; sumAbsR += fabs(R); dF0 += q0; dF1 += q1; dF2 += q2; }
         if (vg && odd) { sumRo += R; sumAbsRo += fabs(R); dF0o += q0; dF1o += q1; dF2o += q2; }
         if (vg) {
+          MGRHD_CHK(oc_cur >= 0 && oc_cur < lim_state);
+          MGRHD_CHK(!t0 || (ftp - scratch >= 0 && ftp - scratch + 2 * ftc < lim_scratch));
           if (P.outer_stop == 1 && !ok) rel_bad = 1;
           if (t0) { ftp[0] = Ft0; ftp[ftc] = Ft1; ftp[2 * ftc] = Ft2; }
           // lagged flux of the next trip, in place
@@ -575,6 +611,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
       for (int i = 0; i < NGB; ++i) {
         const int g = (i << lsh) + subB;
         if (fx && g < Nq) {
+          MGRHD_CHK(sp - smem >= 0 && sp - smem < SS);
           const double vFn = fma(vn0, sp[SL_DA * SS], fma(vn1, sp[SL_DB * SS], vn2 * sp[SL_AG * SS]));
           const double wf = s_tab[(g + 1) * TS + 6] * sp[SL_CHIF * SS] * inv_c;
           const double dWg = fabs(wf * (vFn - sp[SL_VF * SS]));
@@ -624,6 +661,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
       const int g = i * L + sub;
       if (g < Nq) {
         const long long o = (long long)g * stride + fin_cell;
+        MGRHD_CHK(o >= 0 && o * 8 < lim_state);
         S.Erad[o] = S.Erad[o] + smG(SL_R, i);
       }
     }
