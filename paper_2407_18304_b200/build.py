@@ -40,8 +40,9 @@ def needs_build() -> bool:
 
 
 def build(force: bool = False, verbose: bool = False, check: bool = False) -> str:
-    """check=True: the bounds-checked debug build (every shared-memory, state and scratch index is
-    tested where it is used; a violation traps).  Always rebuild without it before timing anything."""
+    """check=True: the bounds-checked debug build (the update kernel's dynamic shared-memory, state and
+    scratch indices are tested where they are used; a violation traps; see DESIGN.md section 11 for what
+    is not covered).  Always rebuild without it before timing anything."""
     if force or check or needs_build():
         cmd = ([_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else [])
                + (["-DMGRHD_BOUNDS_CHECK"] if check else []) + ["-o", LIB] + SOURCES)

@@ -24,9 +24,11 @@
 #pragma once
 #include "mgrhd_planck.cuh"
 
-// Bounds-checked build (python -m paper_2407_18304_b200.build --check): every index into shared
-// memory, the state and the scratch is tested where it is used, and a violation traps.  This stands
-// in for compute-sanitizer, which this pool does not offer; never on in a timed or released build.
+// Bounds-checked build (python -m paper_2407_18304_b200.build --check): the update kernel's indices
+// into its dynamic shared memory, its offsets into the state arrays, its scratch pointers and the
+// cell index are tested where they are used, and a violation traps.  Not covered: s_tab, s_hist,
+// stats[], the __constant__ tables, the other kernels.  A partial stand-in for compute-sanitizer,
+// which this pool does not offer; never on in a timed or released build.
 #ifdef MGRHD_BOUNDS_CHECK
 #define MGRHD_CHK(cond)                                                                       \
   do {                                                                                        \
