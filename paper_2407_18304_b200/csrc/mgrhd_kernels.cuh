@@ -26,8 +26,9 @@
 
 // Bounds-checked build (python -m paper_2407_18304_b200.build --check): the update kernel's indices
 // into its dynamic shared memory, its offsets into the state arrays, its scratch pointers and the
-// cell index are tested where they are used, and a violation traps.  Not covered: s_tab, s_hist,
-// stats[], the __constant__ tables, the other kernels.  A partial stand-in for compute-sanitizer,
+// cell index are tested where they are used, likewise the rows of s_tab, the sign of the histogram
+// bins and the offsets of conserved_totals_kernel; a violation traps.  Not covered: stats[] and the
+// __constant__ tables (compile-time indices).  A partial stand-in for compute-sanitizer,
 // which this pool does not offer; never on in a timed or released build.
 #ifdef MGRHD_BOUNDS_CHECK
 #define MGRHD_CHK(cond)                                                                       \
@@ -241,6 +242,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
     if (sub == 0) {
       cnt_evals += evals;
       cnt_trips += trips;
+      MGRHD_CHK(evals >= 0 && trips >= 0);                       // (the bins are clamped from above only)
       atomicAdd(&s_hist[evals < MGRHD_HIST ? evals : MGRHD_HIST - 1], 1u);
       atomicAdd(&s_hist[MGRHD_HIST + (trips < MGRHD_HIST ? trips : MGRHD_HIST - 1)], 1u);
     }
@@ -371,6 +373,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
           if (evf) { nF0 = ldd(pF0, oc); nF1 = ldd(pF1, oc); nF2 = ldd(pF2, oc); }
           if (fin) nEo = ldd(pE, of);
         }
+        MGRHD_CHK(e >= 1 && Nq <= kMaxG);                          // rows 0..kMaxG of s_tab
         const double2* const row = reinterpret_cast<const double2*>(&s_tab[(e <= Nq ? e : Nq) * TS]);
         const double2 r01 = row[0], r23 = row[1], r45 = row[2], r67 = row[3];
         const double t_nu = r01.x, t_klo = r01.y, t_khi = r23.x, t_kmean = r23.y, t_ikmean = r45.x, t_knum3 = r45.y,
@@ -563,6 +566,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
         const double Enew = Et + R;                               // E_g^(t+1) = E_g^(t) + R_g
         double p0, p1, p2;
         closure_vP(P.closure, Enew, Fk0, Fk1, Fk2, v0, v1, v2, c, p0, p1, p2);
+        MGRHD_CHK(gi >= 0 && gi + 1 <= kMaxG);
         const double w = s_tab[(gi + 1) * TS + 6] * (chisB * s_tab[(gi + 1) * TS + 3]);   // (1 + alpha) chi_E
         const double chiF = g < Nq ? sp[SL_CHIF * SS] : 0.0, A = g < Nq ? sp[SL_AG * SS] : 0.0;
         const double dn = fma(cdt, chiF, 1.0);                    // 1 + c_hat chi_F dt > 0 (guarded in A)
@@ -615,6 +619,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
         if (fx && g < Nq) {
           MGRHD_CHK(sp - smem >= 0 && sp - smem < SS);
           const double vFn = fma(vn0, sp[SL_DA * SS], fma(vn1, sp[SL_DB * SS], vn2 * sp[SL_AG * SS]));
+          MGRHD_CHK(g >= 0 && g + 1 <= kMaxG);
           const double wf = s_tab[(g + 1) * TS + 6] * sp[SL_CHIF * SS] * inv_c;
           const double dWg = fabs(wf * (vFn - sp[SL_VF * SS]));
           if (!ksh && (i & 1)) dWo += dWg; else dW += dWg;
@@ -699,6 +704,7 @@ __global__ void conserved_totals_kernel(const __grid_constant__ StatePtrs S, int
     double sE = 0.0, s0 = 0.0, s1 = 0.0, s2 = 0.0;
     for (int g = 0; g < Nq; ++g) {
       const long long o = (long long)g * stride + i;
+      MGRHD_CHK(o >= 0 && o < (long long)Nq * stride && i < stride);
       sE += S.Erad[o];
       s0 += S.Frad[0][o]; s1 += S.Frad[1][o]; s2 += S.Frad[2][o];
     }
@@ -723,6 +729,7 @@ __global__ void planck_edge_kernel(const double* __restrict__ x, long long n, do
     int fl;
     planck_edge_w(i < n ? x[i] : __longlong_as_double(0x7ff8000000000000ll), (int)(i & 1) * zero, a, b, small, fl);
     if (i < n) {
+      MGRHD_CHK(i >= 0);
       yz[i] = a;
       xi[i] = b;
       is_y[i] = small ? 1 : 0;
