@@ -115,16 +115,26 @@ void fill_planck_tables(PlanckTables& t) {
 std::once_flag g_tables_once[16];  // per device
 cudaError_t g_tables_err[16];
 
+// The host copy of the tables: filled once per process under its own flag (two threads may
+// initialise contexts on different devices at the same time), read-only afterwards.
+const PlanckTables* host_planck_tables() {
+  static PlanckTables t[2];
+  static std::once_flag once;
+  std::call_once(once, []() {
+    fill_planck_tables(t[0]);
+    t[1] = t[0];
+  });
+  return t;
+}
+
 cudaError_t upload_tables_for_current_device() {
   int dev = 0;
   cudaError_t e = cudaGetDevice(&dev);
   if (e != cudaSuccess) return e;
   if (dev < 0 || dev >= 16) return cudaErrorInvalidDevice;
-  std::call_once(g_tables_once[dev], [dev]() {
-    static PlanckTables t[2];
-    fill_planck_tables(t[0]);
-    t[1] = t[0];
-    g_tables_err[dev] = cudaMemcpyToSymbol(mgrhd_c_planck, t, sizeof t);
+  const PlanckTables* t = host_planck_tables();
+  std::call_once(g_tables_once[dev], [dev, t]() {
+    g_tables_err[dev] = cudaMemcpyToSymbol(mgrhd_c_planck, t, 2 * sizeof(PlanckTables));
   });
   return g_tables_err[dev];
 }
@@ -220,7 +230,8 @@ int mgrhd_init(mgrhd_ctx** out, const double* edges, int Nq, const mgrhd_units* 
   for (int g = 0; g < Nq; ++g) {
     if (!(edges[g] >= 0.0) || !(edges[g + 1] > edges[g])) return MGRHD_ERR_EDGES;
     if (m->alpha[g] != 0.0 && (edges[g] == 0.0 || std::isinf(edges[g + 1]))) return MGRHD_ERR_ALPHA;
-    if (!std::isfinite(m->alpha[g]) || !(m->kappa_lo[g] >= 0.0)) return MGRHD_ERR_RANGE;
+    // kappa = 0 makes Eq. 42 singular (E_g = ... /chi_E): rejected, as are inf/NaN
+    if (!std::isfinite(m->alpha[g]) || !(m->kappa_lo[g] > 0.0) || !std::isfinite(m->kappa_lo[g])) return MGRHD_ERR_RANGE;
   }
   mgrhd_ctx* ctx = new (std::nothrow) mgrhd_ctx();
   if (!ctx) return MGRHD_ERR_ARG;
@@ -275,6 +286,8 @@ int mgrhd_init(mgrhd_ctx** out, const double* edges, int Nq, const mgrhd_units* 
 static int check_call(const mgrhd_ctx* ctx, const mgrhd_state* s, long long n, double dt, double c,
                       double chat) {
   if (!ctx || !s || n < 0) return MGRHD_ERR_ARG;
+  int dev = -1;                      // a context belongs to the device that was current in mgrhd_init
+  if (cudaGetDevice(&dev) != cudaSuccess || dev != ctx->device) return MGRHD_ERR_ARG;
   if (!(dt > 0.0) || !(c > 0.0) || !(chat > 0.0) || chat > c) return MGRHD_ERR_RANGE;
   if (n > 0 && (!s->rho || !s->mom[0] || !s->mom[1] || !s->mom[2] || !s->Egas || !s->Erad ||
                 !s->Frad[0] || !s->Frad[1] || !s->Frad[2]))

@@ -93,13 +93,22 @@ __device__ __forceinline__ void closure_vP(int closure, double E, double F0, dou
   // chi = (3 + 4 f^2)/(5 + 2 s), s = sqrt(4 - 3 f^2), equals (5 - 2 s)/3 (multiply through by 5 - 2 s), so
   // (1 - chi)/2 = (s - 1)/3 and (3 chi - 1)/2 = 2 - s: one sqrt, no division
   const double sq = sqrt(fma(-3.0, f2, 4.0));
-  const double r2 = fast_rcp(iso || !(f2u < 1e290) ? 1.0 : f2u);
+  const bool big = !iso && !(f2u < 1e290);       // |F| >> c E (f is clamped to 1): f^2 or t itself overflows
+  const double r2 = fast_rcp(iso || big ? 1.0 : f2u);
   const double tv = fma(t0, v0, fma(t1, v1, t2 * v2));
   const double a = iso ? 1.0 / 3.0 : (sq - 1.0) * (1.0 / 3.0);
   const double b = (2.0 - sq) * tv * r2;
   p0 = E * fma(a, v0, iso ? 0.0 : b * t0);       // (t may be inf/NaN on isotropic lanes: selected away)
   p1 = E * fma(a, v1, iso ? 0.0 : b * t1);
   p2 = E * fma(a, v2, iso ? 0.0 : b * t2);
+  if (__any_sync(0xffffffffu, big)) {            // warp-uniform and practically never taken
+    // free-streaming limit f = 1 (chi = 1, P = E n n): n from F scaled by its largest component,
+    // so that n (n.v) is formed finitely whatever F/(cE) is (E ~ 1e-320 beside F ~ 1e-150)
+    const double m = fmax(fabs(F0), fmax(fabs(F1), fabs(F2)));
+    const double u0 = F0 / m, u1 = F1 / m, u2 = F2 / m;
+    const double uv = fma(u0, v0, fma(u1, v1, u2 * v2)) / fma(u0, u0, fma(u1, u1, u2 * u2));
+    if (big) { p0 = E * (uv * u0); p1 = E * (uv * u1); p2 = E * (uv * u2); }
+  }
 }
 
 // Lane phases of the flattened iteration.
@@ -149,7 +158,6 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
   double* const scratch = scratch0 + kScratchHead;
   extern __shared__ double smem[];
   __shared__ unsigned int s_hist[2 * MGRHD_HIST];
-  __shared__ unsigned int s_cnt[8];   // per-CTA counters of rare events, indexed by StatSlot (registers are scarce)
   // Per-edge table rows in shared memory, row e = {nu_e, and for the group below edge e: k_lo, k_hi,
   // k_mean, 1/k_mean, (4+alpha) k_mean, 1+alpha, (1+alpha)/k_mean}.  The L lanes of a cell read L neighbouring rows per step
   // (broadcast within equal `sub`), which would otherwise be lane-indexed constant loads that miss
@@ -157,7 +165,6 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
   constexpr int TS = 10;   // row stride in doubles: 80 B puts the L rows of a step on distinct banks
   __shared__ __align__(16) double s_tab[(kMaxG + 1) * TS];
   for (int t = threadIdx.x; t < 2 * MGRHD_HIST; t += THREADS) s_hist[t] = 0u;
-  if (threadIdx.x < 8) s_cnt[threadIdx.x] = 0u;
   for (int r = threadIdx.x; r <= P.Nq; r += THREADS) {
     const int g = r > 0 ? r - 1 : 0;
     s_tab[r * TS + 0] = P.nu[r];

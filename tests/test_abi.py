@@ -67,6 +67,9 @@ def test_init_argument_errors(binding):
         _init(binding, e, k, a, gamma=1.0)
     with pytest.raises(binding.MgrhdError, match="MGRHD_ERR_RANGE"):
         _init(binding, e, k, a, a_rad=0.0)
+    for bad_k in (0.0, -1.0, np.inf, np.nan):           # kappa = 0 makes Eq. 42 singular (1/chi_E)
+        with pytest.raises(binding.MgrhdError, match="MGRHD_ERR_RANGE"):
+            _init(binding, e, np.array([1.0, bad_k]), a)
     with pytest.raises(binding.MgrhdError, match="MGRHD_ERR_ARG"):
         _init(binding, e, k, a, closure=2)
     with pytest.raises(binding.MgrhdError, match="MGRHD_ERR_ARG"):

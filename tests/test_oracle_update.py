@@ -192,6 +192,9 @@ def _brute_force_residual(p, x):
         Db = aT4 * (mp_Xi(xhi) - mp_Xi(xlo))
         D = aT4 * (chihi * mp_Xi(xhi) - chilo * mp_Xi(xlo))
         chiF = ((chiB + chiE / 3) * Bt + (al * chiE * Bt - D) / 3) / (mp.mpf(4) / 3 * Bt - Db / 3)   # Eq. 27
+        if g in p.get("chiF_is_chiE", ()):       # reading S8(ii): groups in which 1 + c_hat chi_F dt <= 0
+            assert 1 + chat * chiF * dt <= 0
+            chiF = chiE
         Fn = mp.sqrt(sum(f ** 2 for f in F[g]))
         f = Fn / (c * E[g])
         chiEdd = (3 + 4 * f ** 2) / (5 + 2 * mp.sqrt(4 - 3 * f ** 2))                     # Levermore 1984
