@@ -9,6 +9,7 @@ from .oracle import (  # noqa: F401
     build,
     chi_flux,
     chi_mean,
+    free_slopes,
     arrowhead_solve,
     lu_solve,
     planck_dY,

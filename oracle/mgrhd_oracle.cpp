@@ -25,8 +25,14 @@
 // diffusion flux, conservation to round-off, the grey (Nq=1) limit of
 // Eq. 5-6, the scalar monotone energy balance by bisection, a brute-force
 // high-precision solve of the full (4+4Nq) system, arrowhead vs dense LU.
-// PPL free-slope (Appendix A) is not implemented here: parity unpinned /
-// out of scope this round.
+// Round 2 additions (each pinned in tests/test_oracle_next.py): the optional
+// source term S_g; opacities evaluated at the
+// trial temperature -- kappa_g (T/T_ref)^p and edge values
+// tabulated in T with alpha from Eq. 20; the PPL free-slope
+// spectrum fit of Appendix A.  The free-slope ITERATION is
+// "parity unpinned" beyond its fixed point (brute-force solve) and the
+// special cases listed in DESIGN.md: the paper does not say from which
+// iterate of E_g the slope alpha_E is taken (reading S20).
 //
 // Notation (energy-density units, so 4*pi/c never appears):
 //   x      = h nu / (k_B T)
@@ -142,9 +148,37 @@ double powint(double lnr, double p) {
   return std::expm1(z) / p;
 }
 
+// minmod of Eq. A2: zero when the one-sided slopes differ in sign, else the one of smaller magnitude.
+double minmod(double a, double b) {
+  if (a * b <= 0.0) return 0.0;
+  return std::fabs(a) < std::fabs(b) ? a : b;
+}
+
 }  // namespace
 
 extern "C" {
+
+// Appendix A, Eq. A1-A2: powerlaw indices alpha_{Q,g} of a radiation quantity from
+// its group integrals Q[Nq].  Qbar_g = Q_g/(nu_g+ - nu_g-), nubar_g = sqrt(nu_g+ nu_g-),
+// s_{g+1/2} = ln(Qbar_{g+1}/Qbar_g)/ln(nubar_{g+1}/nubar_g), alpha_g = minmod(s_{g-1/2}, s_{g+1/2});
+// the two edge groups get -1.  Reading S21 (paper silent): a group whose own or whose neighbour's Q is
+// not positive (the logarithm does not exist), or whose group structure has a zero or infinite edge,
+// also gets -1, the fixed-slope value.
+void oracle_free_slopes(int Nq, const double* edges, const double* Q, double* alphaQ) {
+  for (int g = 0; g < Nq; ++g) alphaQ[g] = -1.0;
+  for (int g = 1; g + 1 < Nq; ++g) {
+    bool ok = true;
+    double s[2];
+    for (int k = 0; k < 2 && ok; ++k) {
+      const int a = g - 1 + k, b = g + k;                    // the pair (a, b) = (g-1, g) then (g, g+1)
+      const double wa = edges[a + 1] - edges[a], wb = edges[b + 1] - edges[b];
+      if (!(Q[a] > 0.0) || !(Q[b] > 0.0) || !(edges[a] > 0.0) || !std::isfinite(edges[b + 1])) { ok = false; break; }
+      const double na = std::sqrt(edges[a + 1] * edges[a]), nb = std::sqrt(edges[b + 1] * edges[b]);
+      s[k] = std::log((Q[b] / wb) / (Q[a] / wa)) / std::log(nb / na);     // Eq. A1
+    }
+    if (ok) alphaQ[g] = minmod(s[0], s[1]);                                  // Eq. A2
+  }
+}
 
 // Eq. 30 (reading S1): chi_{0Q,g} = chi_{0,g-} * [ (r^(aQ+1)-1)/(aQ+1) ]^-1
 //                                              * [ (r^(ax+aQ+1)-1)/(ax+aQ+1) ].
@@ -250,6 +284,16 @@ typedef struct {
   double outer_tol;         // 1e-13 of PAPER.md:465
   int outer_stop;           // 0 paper rule; 1 paper rule AND relative change of F_g, rho v (S10)
   double outer_rel_tol;     // 1e-12 (S10), used when outer_stop == 1
+  // ---- round 2 ----
+  int spectrum;             // 0 PPL fixed slope alpha_Q = -1; 1 free slope (Appendix A)
+  int opacity_kind;         // 0 table (kappa_lo, alpha) independent of T
+                            // 1 kappa_lo[g] (T/T_ref)^p_T, alpha as given
+                            // 2 ln kappa tabulated at the Nq+1 EDGES on a uniform grid in ln T, alpha_g from the
+                            //   two edge values of the group at the trial T (Eq. 20)
+  double T_ref, p_T;        // kind 1
+  int NT;                   // kind 2: temperatures in the table
+  double lnT0, dlnT;        //         T_j = exp(lnT0 + j dlnT)
+  const double* lnk_edge;   //         [Nq+1][NT] ln of the specific opacity at edge e, temperature j
 } oracle_model;
 
 enum { ORACLE_HIST = 64 };
@@ -273,13 +317,31 @@ namespace {
 inline double norm3(const double a[3]) { return std::sqrt(a[0] * a[0] + a[1] * a[1] + a[2] * a[2]); }
 
 // One cell.  E[g], F[i][g] are the cell's group arrays; all updated in place.
+// Specific opacity at edge e at temperature T for opacity_kind 2: linear interpolation of ln kappa in ln T
+// between the two neighbouring table temperatures, the end values outside the table (reading S19).
+double table_kappa(const oracle_model& m, int e, double T) {
+  double u = (std::log(T) - m.lnT0) / m.dlnT;
+  if (!(u > 0.0)) u = 0.0;
+  if (u > (double)(m.NT - 1)) u = (double)(m.NT - 1);
+  int j = (int)u;
+  if (j > m.NT - 2) j = m.NT - 2;
+  if (j < 0) j = 0;
+  const double w = (m.NT > 1) ? u - (double)j : 0.0;
+  const double* row = m.lnk_edge + (size_t)e * m.NT;
+  const double lnk = (m.NT > 1) ? (1.0 - w) * row[j] + w * row[j + 1] : row[0];
+  return std::exp(lnk);
+}
+
+// Ssrc: the cell's S_g [Nq], or null for S_g = 0.
 void update_cell(const oracle_model& m, double dt, double c, double chat,
                  double rho, double kscale, double mom[3], double& Egas,
-                 double* E, double* F0, double* F1, double* F2, oracle_stats& st) {
+                 double* E, double* F0, double* F1, double* F2, const double* Ssrc, oracle_stats& st) {
   const int Nq = m.Nq;
   double* Fp[3] = {F0, F1, F2};
   std::vector<double> chi_lo(Nq), chi_hi(Nq), chiB(Nq), chiE(Nq), R(Nq, 0.0), Bt(Nq), Db(Nq), D(Nq),
-      dBdT(Nq), chiF(Nq), W(Nq), Eg(Nq), FR(Nq), Enew(Nq), vF(Nq), xe(Nq + 1), Xi(Nq + 1);
+      dBdT(Nq), chiF(Nq), W(Nq), Eg(Nq), FR(Nq), Enew(Nq), vF(Nq), xe(Nq + 1), Xi(Nq + 1), alpha(Nq), Sg(Nq, 0.0),
+      alphaB(Nq, -1.0), alphaE(Nq, -1.0), Ecur(Nq), chi_edge(Nq + 1);
+  if (Ssrc) Sg.assign(Ssrc, Ssrc + Nq);
   std::vector<double> Ft[3], Fk[3], Fnew[3];
   for (int i = 0; i < 3; ++i) { Ft[i].assign(Fp[i], Fp[i] + Nq); Fk[i] = Ft[i]; Fnew[i] = Ft[i]; }
   const std::vector<double> Et(E, E + Nq);
@@ -287,22 +349,45 @@ void update_cell(const oracle_model& m, double dt, double c, double chat,
   const double mom_t[3] = {mom[0], mom[1], mom[2]};
   double mom_k[3] = {mom[0], mom[1], mom[2]}, mom_new[3] = {mom[0], mom[1], mom[2]};
 
-  // O0: opacities at the group edges (Eq. 19) and group means (Eq. 30, alpha_Q = -1)
-  for (int g = 0; g < Nq; ++g) {
-    chi_lo[g] = rho * kscale * m.kappa_lo[g];
-    if (m.alpha[g] == 0.0) {
-      chi_hi[g] = chi_lo[g];
-      chiB[g] = chiE[g] = chi_lo[g];
-    } else {
-      double lnr = std::log(m.edges[g + 1] / m.edges[g]);
-      chi_hi[g] = chi_lo[g] * std::exp(m.alpha[g] * lnr);
-      chiB[g] = oracle_chi_mean(chi_lo[g], lnr, m.alpha[g], -1.0);
-      chiE[g] = oracle_chi_mean(chi_lo[g], lnr, m.alpha[g], -1.0);  // same method for both
+  // O0/a3: opacities at the group edges (Eq. 19, 20) and group means (Eq. 30) at temperature T and, for the
+  // free-slope spectrum, at the current iterate of the radiation energies.  For the T-independent table with
+  // the fixed slope this is the same for every trial T (and is then what round 1 evaluated once per cell).
+  auto opacities = [&](double T, const std::vector<double>& Bt_now, const std::vector<double>& E_now) {
+    if (m.opacity_kind == 2)
+      for (int e = 0; e <= Nq; ++e) chi_edge[e] = rho * kscale * table_kappa(m, e, T);
+    if (m.spectrum == 1) {                                          // Appendix A, for B_g and for E_g alike
+      oracle_free_slopes(Nq, m.edges, Bt_now.data(), alphaB.data());
+      oracle_free_slopes(Nq, m.edges, E_now.data(), alphaE.data());
     }
-  }
-  double sumEt = 0.0;
-  for (int g = 0; g < Nq; ++g) sumEt += Et[g];
-  const double Etot = Egas_t + (chat / c) * sumEt;                  // Eq. 50 as printed (S4), S_g = 0
+    for (int g = 0; g < Nq; ++g) {
+      double lnr = 0.0;
+      if (m.opacity_kind == 2) {
+        lnr = std::log(m.edges[g + 1] / m.edges[g]);
+        chi_lo[g] = chi_edge[g];
+        chi_hi[g] = chi_edge[g + 1];
+        alpha[g] = std::log(chi_hi[g] / chi_lo[g]) / lnr;           // Eq. 20
+      } else {
+        alpha[g] = m.alpha[g];
+        chi_lo[g] = rho * kscale * m.kappa_lo[g];
+        if (m.opacity_kind == 1) chi_lo[g] *= std::pow(T / m.T_ref, m.p_T);
+        if (alpha[g] != 0.0) {
+          lnr = std::log(m.edges[g + 1] / m.edges[g]);
+          chi_hi[g] = chi_lo[g] * std::exp(alpha[g] * lnr);         // Eq. 19 at nu_g+
+        } else {
+          chi_hi[g] = chi_lo[g];
+        }
+      }
+      if (alpha[g] == 0.0) {
+        chiB[g] = chiE[g] = chi_lo[g];                              // PC, Eq. 17
+      } else {
+        chiB[g] = oracle_chi_mean(chi_lo[g], lnr, alpha[g], alphaB[g]);   // Eq. 30; alpha_Q = -1 unless free slope
+        chiE[g] = oracle_chi_mean(chi_lo[g], lnr, alpha[g], alphaE[g]);   // same method for both
+      }
+    }
+  };
+  double sumEt = 0.0, sumS = 0.0;
+  for (int g = 0; g < Nq; ++g) { sumEt += Et[g]; sumS += Sg[g]; }
+  const double Etot = Egas_t + (chat / c) * (sumEt + sumS);         // Eq. 50 as printed (S4)
   const double Cv = rho * m.k_B / ((m.gamma - 1.0) * m.mean_mass);  // S15
 
   double Egs = Egas_t;          // Newton iterate E_gas*
@@ -327,24 +412,30 @@ void update_cell(const oracle_model& m, double dt, double c, double chat,
         Xi[e] = oracle_planck_Xi(xe[e]);
       }
       double sumR = 0.0, sumAbsFR = 0.0;
+      // O3 (first half): group Planck integrals (Eq. 11); a3: opacities at this trial T; the free-slope fit
+      // takes E_g at the current iterate, E_g^(t) + R_g + S_g (reading S20)
       for (int g = 0; g < Nq; ++g) {
-        // O3: group Planck integral and Doppler boundary terms (Eq. 11, 18, 22)
         Bt[g] = aT4 * oracle_planck_dY(xe[g], xe[g + 1]);
+        Ecur[g] = Et[g] + R[g] + Sg[g];
+      }
+      opacities(T, Bt, Ecur);
+      for (int g = 0; g < Nq; ++g) {
+        // O3: Doppler boundary terms (Eq. 18, 22)
         Db[g] = aT4 * (Xi[g + 1] - Xi[g]);
         D[g] = aT4 * (chi_hi[g] * Xi[g + 1] - chi_lo[g] * Xi[g]);
         dBdT[g] = (4.0 * Bt[g] - Db[g]) / T;
         // O4: flux-mean opacity (Eq. 27) and the work term of Eq. 21
         int guard = 0;
-        chiF[g] = oracle_chi_flux(chiB[g], chiE[g], m.alpha[g], chi_lo[g], Bt[g], Db[g], D[g], aT4, &guard);
+        chiF[g] = oracle_chi_flux(chiB[g], chiE[g], alpha[g], chi_lo[g], Bt[g], Db[g], D[g], aT4, &guard);
         if (guard && newton_evals == 0) st.n_chiF_guard++;
         if (!(1.0 + chat * chiF[g] * dt > 0.0)) {                  // S8(ii)
           if (newton_evals == 0) st.n_denominator_nonpositive++;
           chiF[g] = chiE[g];
         }
-        W[g] = (1.0 + m.alpha[g]) * chiF[g] * vF[g] / c;
-        // O5: Eq. 42 (reading S2) solved for E_g; residuals of Eq. 41 with S_g = 0
+        W[g] = (1.0 + alpha[g]) * chiF[g] * vF[g] / c;
+        // O5: Eq. 42 (reading S2) solved for E_g; residuals of Eq. 41
         Eg[g] = (chiB[g] / chiE[g]) * Bt[g] + W[g] / (c * chiE[g]) - R[g] / (chat * dt * chiE[g]);
-        FR[g] = Eg[g] - Et[g] - R[g];
+        FR[g] = Eg[g] - Et[g] - (R[g] + Sg[g]);
         sumR += R[g];
         sumAbsFR += std::fabs(FR[g]);
       }
@@ -377,7 +468,7 @@ void update_cell(const oracle_model& m, double dt, double c, double chat,
 
     // O8: energy commit
     double sumR = 0.0;
-    for (int g = 0; g < Nq; ++g) { Enew[g] = Et[g] + R[g]; sumR += R[g]; }
+    for (int g = 0; g < Nq; ++g) { Enew[g] = Et[g] + R[g] + Sg[g]; sumR += R[g]; }
     Egas_new = Egas_t - (c / chat) * sumR;
 
     // O9: flux update with the lagged velocity (Eq. 51); O10: gas momentum (Eq. 52)
@@ -386,7 +477,7 @@ void update_cell(const oracle_model& m, double dt, double c, double chat,
       double Fg[3] = {Fk[0][g], Fk[1][g], Fk[2][g]}, vP[3];
       oracle_vP(m.closure, Enew[g], Fg, v, c, vP);
       for (int i = 0; i < 3; ++i) {
-        double src = v[i] * (chiB[g] * Bt[g] - D[g] / 3.0) + (1.0 + m.alpha[g]) * chiE[g] * vP[i];
+        double src = v[i] * (chiB[g] * Bt[g] - D[g] / 3.0) + (1.0 + alpha[g]) * chiE[g] * vP[i];
         Fnew[i][g] = (Ft[i][g] + chat * dt * src) / (1.0 + chat * chiF[g] * dt);
         dFsum[i] += Fnew[i][g] - Ft[i][g];
       }
@@ -400,7 +491,7 @@ void update_cell(const oracle_model& m, double dt, double c, double chat,
     bool rel_ok = true;
     for (int g = 0; g < Nq; ++g) {
       double vFn = vn[0] * Fnew[0][g] + vn[1] * Fnew[1][g] + vn[2] * Fnew[2][g];
-      double Wn = (1.0 + m.alpha[g]) * chiF[g] * vFn / c;
+      double Wn = (1.0 + alpha[g]) * chiF[g] * vFn / c;
       dW += std::fabs(Wn - W[g]);
       sumAbsR += std::fabs(R[g]);
       if (m.outer_stop == 1) {
@@ -439,25 +530,34 @@ void update_cell(const oracle_model& m, double dt, double c, double chat,
 extern "C" {
 
 // Host arrays, SoA, updated in place (rho, kappa_scale read-only):
-//   rho[n], mom0/1/2[n], Egas[n], Erad[Nq][n], Frad0/1/2[Nq][n], kappa_scale[n] or NULL.
+//   rho[n], mom0/1/2[n], Egas[n], Erad[Nq][n], Frad0/1/2[Nq][n], kappa_scale[n] or NULL,
+//   Srad[Nq][n] or NULL (the source term S_g of Eq. 41; read only).
 // Returns 0, or a negative code for an argument error.
 int oracle_source_update(const oracle_model* m, long long n, const double* rho,
                          double* mom0, double* mom1, double* mom2, double* Egas,
                          double* Erad, double* Frad0, double* Frad1, double* Frad2,
-                         const double* kappa_scale, double dt, double c, double chat,
+                         const double* kappa_scale, const double* Srad, double dt, double c, double chat,
                          oracle_stats* stats) {
-  if (!m || m->Nq < 1 || !m->edges || !m->kappa_lo || !m->alpha) return -1;
+  if (!m || m->Nq < 1 || !m->edges) return -1;
+  if (m->opacity_kind < 0 || m->opacity_kind > 2 || m->spectrum < 0 || m->spectrum > 1) return -1;
+  if (m->opacity_kind != 2 && (!m->kappa_lo || !m->alpha)) return -1;
+  if (m->opacity_kind == 2 && (!m->lnk_edge || m->NT < 1 || (m->NT > 1 && !(m->dlnT > 0.0)))) return -1;
+  if (m->opacity_kind == 1 && !(m->T_ref > 0.0)) return -2;
   if (!(dt > 0.0) || !(c > 0.0) || !(chat > 0.0) || chat > c) return -2;
   for (int g = 0; g < m->Nq; ++g) {
     if (!(m->edges[g + 1] > m->edges[g]) || m->edges[g] < 0.0) return -3;
-    if (m->alpha[g] != 0.0 && (m->edges[g] == 0.0 || std::isinf(m->edges[g + 1]))) return -4;
+    const bool open_group = m->edges[g] == 0.0 || std::isinf(m->edges[g + 1]);
+    if (m->opacity_kind != 2 && m->alpha[g] != 0.0 && open_group) return -4;
+    if (m->opacity_kind == 2 && open_group) return -4;      // Eq. 20 needs both edge values of every group
+    if (m->opacity_kind != 2 && !(m->kappa_lo[g] > 0.0)) return -2;   // kappa = 0 makes Eq. 42 singular
   }
   oracle_stats st;
   std::memset(&st, 0, sizeof st);
   const int Nq = m->Nq;
-  std::vector<double> E(Nq), F0(Nq), F1(Nq), F2(Nq);
+  std::vector<double> E(Nq), F0(Nq), F1(Nq), F2(Nq), Sc(Nq);
   for (long long i = 0; i < n; ++i) {
     for (int g = 0; g < Nq; ++g) {
+      if (Srad) Sc[g] = Srad[(size_t)g * n + i];
       E[g] = Erad[(size_t)g * n + i];
       F0[g] = Frad0[(size_t)g * n + i];
       F1[g] = Frad1[(size_t)g * n + i];
@@ -466,7 +566,7 @@ int oracle_source_update(const oracle_model* m, long long n, const double* rho,
     double mom[3] = {mom0[i], mom1[i], mom2[i]};
     double eg = Egas[i];
     update_cell(*m, dt, c, chat, rho[i], kappa_scale ? kappa_scale[i] : 1.0, mom, eg,
-                E.data(), F0.data(), F1.data(), F2.data(), st);
+                E.data(), F0.data(), F1.data(), F2.data(), Srad ? Sc.data() : nullptr, st);
     mom0[i] = mom[0]; mom1[i] = mom[1]; mom2[i] = mom[2];
     Egas[i] = eg;
     for (int g = 0; g < Nq; ++g) {

@@ -46,6 +46,14 @@ class _CModel(ctypes.Structure):
         ("outer_tol", ctypes.c_double),
         ("outer_stop", ctypes.c_int),
         ("outer_rel_tol", ctypes.c_double),
+        ("spectrum", ctypes.c_int),
+        ("opacity_kind", ctypes.c_int),
+        ("T_ref", ctypes.c_double),
+        ("p_T", ctypes.c_double),
+        ("NT", ctypes.c_int),
+        ("lnT0", ctypes.c_double),
+        ("dlnT", ctypes.c_double),
+        ("lnk_edge", ctypes.POINTER(ctypes.c_double)),
     ]
 
 
@@ -87,8 +95,10 @@ def _load():
         L.oracle_arrowhead_solve.argtypes = [ctypes.c_int, d, dp, dp, dp, dp, dp]
         L.oracle_source_update.restype = ctypes.c_int
         L.oracle_source_update.argtypes = (
-            [ctypes.POINTER(_CModel), ctypes.c_longlong] + [dp] * 10 + [d, d, d, ctypes.POINTER(_CStats)]
+            [ctypes.POINTER(_CModel), ctypes.c_longlong] + [dp] * 11 + [d, d, d, ctypes.POINTER(_CStats)]
         )
+        L.oracle_free_slopes.restype = None
+        L.oracle_free_slopes.argtypes = [ctypes.c_int, dp, dp, dp]
         _lib = L
     return _lib
 
@@ -136,6 +146,14 @@ def vP(closure, E, F, v, c):
     return out
 
 
+def free_slopes(edges, Q) -> np.ndarray:
+    """Appendix A (Eq. A1-A2): alpha_{Q,g} from the group integrals Q[Nq]."""
+    e, q = _arr(edges), _arr(Q)
+    out = np.empty(q.shape[0])
+    _load().oracle_free_slopes(q.shape[0], _p(e), _p(q), _p(out))
+    return out
+
+
 def lu_solve(A, b):
     A = _arr(A).copy()
     b = _arr(b).copy()
@@ -174,16 +192,27 @@ class OracleModel:
     outer_tol: float = 1e-13
     outer_stop: int = 1
     outer_rel_tol: float = 1e-12
+    spectrum: int = 0            # 0 fixed slope alpha_Q = -1; 1 free slope (Appendix A)
+    opacity_kind: int = 0        # 0 table; 1 kappa_lo (T/T_ref)^p_T; 2 ln kappa at the edges tabulated in ln T (Eq. 20)
+    T_ref: float = 1.0
+    p_T: float = 0.0
+    lnT0: float = 0.0
+    dlnT: float = 1.0
+    lnk_edge: np.ndarray | None = None   # [Nq+1, NT] for opacity_kind 2
     _keep: list = field(default_factory=list, repr=False)
 
     def _c(self) -> _CModel:
         e, k, a = _arr(self.edges), _arr(self.kappa_lo), _arr(self.alpha)
         assert e.shape[0] == k.shape[0] + 1 == a.shape[0] + 1
-        self._keep = [e, k, a]
+        t = None if self.lnk_edge is None else _arr(self.lnk_edge)
+        if t is not None:
+            assert t.ndim == 2 and t.shape[0] == e.shape[0]
+        self._keep = [e, k, a, t]
         return _CModel(
             k.shape[0], _p(e), self.a_rad, self.k_B, self.h_planck, self.mean_mass, self.gamma, _p(k), _p(a),
             self.closure, self.newton_tol, self.newton_maxit, self.outer_maxit, self.outer_tol,
-            self.outer_stop, self.outer_rel_tol,
+            self.outer_stop, self.outer_rel_tol, self.spectrum, self.opacity_kind, self.T_ref, self.p_T,
+            0 if t is None else t.shape[1], self.lnT0, self.dlnT, None if t is None else _p(t),
         )
 
 
@@ -203,12 +232,16 @@ def source_update(model: OracleModel, state: dict, dt: float, c: float, c_hat: f
     ks = state.get("kappa_scale")
     if ks is not None:
         assert ks.dtype == np.float64 and ks.flags.c_contiguous and ks.shape == (n,)
+    sr = state.get("Srad")
+    if sr is not None:
+        assert sr.dtype == np.float64 and sr.flags.c_contiguous and sr.shape == (Nq, n)
     st = _CStats()
     rc = _load().oracle_source_update(
         ctypes.byref(cm), n, _p(state["rho"]),
         _p(state["mom"][0]), _p(state["mom"][1]), _p(state["mom"][2]), _p(state["Egas"]), _p(state["Erad"]),
         _p(state["Frad"][0]), _p(state["Frad"][1]), _p(state["Frad"][2]),
-        _p(ks) if ks is not None else None, float(dt), float(c), float(c_hat), ctypes.byref(st),
+        _p(ks) if ks is not None else None, _p(sr) if sr is not None else None,
+        float(dt), float(c), float(c_hat), ctypes.byref(st),
     )
     if rc != 0:
         raise ValueError(f"oracle_source_update: argument error {rc}")

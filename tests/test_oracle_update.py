@@ -168,6 +168,25 @@ def test_inner_solve_matches_bisection_of_scalar_balance(oracle_lib):
 # ---------------------------------------------------------------------------
 # whole update: brute-force solve of the full implicit system in 30-digit arithmetic
 # ---------------------------------------------------------------------------
+def _mp_eq30(chilo, lnr, a_chi, a_Q):
+    """Eq. 30 (reading S1) typed out: chi_lo [(r^(aQ+1)-1)/(aQ+1)]^-1 [(r^(ax+aQ+1)-1)/(ax+aQ+1)], ln r at exponent 0."""
+    br = lambda q: lnr if q == 0 else mp.expm1(q * lnr) / q  # noqa: E731
+    return chilo * br(a_chi + a_Q + 1) / br(a_Q + 1)
+
+
+def _mp_free_slopes(edges, Q):
+    """Eq. A1-A2 typed out in mpmath; edge groups -1."""
+    Nq = len(Q)
+    qb = [Q[g] / (edges[g + 1] - edges[g]) for g in range(Nq)]
+    nb = [mp.sqrt(edges[g + 1] * edges[g]) for g in range(Nq)]
+    out = [mp.mpf(-1)] * Nq
+    for g in range(1, Nq - 1):
+        sm = mp.log(qb[g] / qb[g - 1]) / mp.log(nb[g] / nb[g - 1])
+        sp = mp.log(qb[g + 1] / qb[g]) / mp.log(nb[g + 1] / nb[g])
+        out[g] = mp.mpf(0) if sm * sp <= 0 else (sm if abs(sm) < abs(sp) else sp)
+    return out
+
+
 def _brute_force_residual(p, x):
     """Residuals of Eq. 37-40 with the four-force of Eq. 21-22 at the NEW state, opacity means from Eq. 30
     (alpha_Q = -1), chi_F from Eq. 27, M1 closure group by group.  Typed from the paper, in mpmath."""
@@ -182,13 +201,22 @@ def _brute_force_residual(p, x):
     res = [None] * (4 + 4 * Nq)
     sumG0c = mp.mpf(0)
     sumG = [mp.mpf(0)] * 3
+    # options of the round-2 extensions (absent = the round-1 system):
+    #   "S": source terms S_g;  "pT","Tref": chi(T) = chi (T/Tref)^pT at the NEW temperature;
+    #   "free": alpha_Q of Appendix A recomputed from the NEW B_g and E_g
+    S = p.get("S", [mp.mpf(0)] * Nq)
+    tscale = (T / p["Tref"]) ** p["pT"] if "pT" in p else mp.mpf(1)
+    Bts = [aT4 * mp_dY(p["h"] * p["edges"][g] / (p["kB"] * T), p["h"] * p["edges"][g + 1] / (p["kB"] * T)) for g in range(Nq)]
+    aB = aE = [mp.mpf(-1)] * Nq
+    if p.get("free"):
+        aB, aE = _mp_free_slopes(p["edges"], Bts), _mp_free_slopes(p["edges"], E)
     for g in range(Nq):
-        nlo, nhi, al, chilo = p["edges"][g], p["edges"][g + 1], p["alpha"][g], p["chi_lo"][g]
+        nlo, nhi, al, chilo = p["edges"][g], p["edges"][g + 1], p["alpha"][g], p["chi_lo"][g] * tscale
         lnr = mp.log(nhi / nlo) if al != 0 else mp.mpf(1)
         chihi = chilo * mp.exp(al * lnr) if al != 0 else chilo
-        chiB = chiE = chilo * mp.expm1(al * lnr) / (al * lnr) if al != 0 else chilo     # Eq. 30, alpha_Q = -1
+        chiB, chiE = (_mp_eq30(chilo, lnr, al, aB[g]), _mp_eq30(chilo, lnr, al, aE[g])) if al != 0 else (chilo, chilo)
         xlo, xhi = p["h"] * nlo / (p["kB"] * T), p["h"] * nhi / (p["kB"] * T)
-        Bt = aT4 * mp_dY(xlo, xhi)
+        Bt = Bts[g]
         Db = aT4 * (mp_Xi(xhi) - mp_Xi(xlo))
         D = aT4 * (chihi * mp_Xi(xhi) - chilo * mp_Xi(xlo))
         chiF = ((chiB + chiE / 3) * Bt + (al * chiE * Bt - D) / 3) / (mp.mpf(4) / 3 * Bt - Db / 3)   # Eq. 27
@@ -205,7 +233,7 @@ def _brute_force_residual(p, x):
         # -c G0_g (Eq. 21) and -G^i_g (Eq. 22), in energy-density units (4 pi B_g = c Bt)
         mcG0 = c * chiB * Bt - c * chiE * E[g] + (1 + al) * chiF * vF / c
         mG = [-chiF * F[g][i] / c + v[i] * (chiB * Bt - D / 3) / c + (1 + al) * chiE * vP[i] / c for i in range(3)]
-        res[4 + g] = E[g] - p["E0"][g] - (chat / c) * dt * mcG0                           # Eq. 38
+        res[4 + g] = E[g] - p["E0"][g] - (chat / c) * dt * mcG0 - S[g]                    # Eq. 38 (+ S_g, Eq. 41)
         for i in range(3):
             res[4 + Nq + 3 * g + i] = F[g][i] - p["F0"][g][i] - chat * c * dt * mG[i]      # Eq. 40
             sumG[i] += -mG[i]
