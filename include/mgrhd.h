@@ -31,9 +31,9 @@ extern "C" {
 enum {
   MGRHD_OK = 0,
   MGRHD_ERR_ARG = -1,        /* null pointer, Nq out of range, ncells < 0, bad enum value      */
-  MGRHD_ERR_RANGE = -2,      /* dt <= 0, c <= 0, c_hat <= 0 or c_hat > c, non-positive units    */
+  MGRHD_ERR_RANGE = -2,      /* dt <= 0, c <= 0, c_hat <= 0 or c_hat > c, non-positive units or opacities */
   MGRHD_ERR_EDGES = -3,      /* edges not strictly ascending, negative, or NaN                  */
-  MGRHD_ERR_ALPHA = -4,      /* alpha != 0 in a group whose edge is 0 or +inf (Eq. 19 undefined) */
+  MGRHD_ERR_ALPHA = -4,      /* alpha != 0 (or opacity_kind 2) in a group whose edge is 0 or +inf (Eq. 19, 20 undefined) */
   MGRHD_ERR_CUDA = -5        /* CUDA runtime failure; mgrhd_last_error() has the text           */
 };
 
@@ -53,18 +53,32 @@ typedef struct {
   const double *kappa_lo;  /* [Nq] specific opacity at each group's LOWER edge (Eq. 19)        */
   const double *alpha;     /* [Nq] in-group power-law slope alpha_{chi0,g}; 0 => PC (Eq. 17)   */
   int closure;             /* 0 = Levermore/M1, 1 = Eddington P = E/3 I (:603)  */
-  int spectrum;            /* 0 = PPL fixed slope alpha_Q = -1; others rejected */
+  int spectrum;            /* 0 = PPL fixed slope alpha_Q = -1 (the paper's favoured method);
+                              1 = PPL free slope: alpha_B,g and alpha_E,g refitted at every Newton evaluation from
+                              the group integrals B_g(T) and E_g^(t) + R_g + S_g by Eq. A1-A2,
+                              both means from Eq. 30                                           */
   double newton_tol;       /* epsilon of Eq. 49 (paper default 1e-11)            */
   int newton_maxit;        /* cap on Newton steps per outer trip (paper silent; 50)            */
   int outer_maxit;         /* cap on outer trips (paper silent; 50)                            */
   double outer_tol;        /* 1e-13 of PAPER.md:465                                            */
   int outer_stop;          /* 0 = paper rule only; 1 = also |dF_g|<=rel*|F_g|, |d rho v|<=rel*|rho v| */
   double outer_rel_tol;    /* rel of outer_stop == 1 (1e-12)                                   */
+  /* ---- opacities that depend on the gas temperature: evaluated at every trial T of the Newton iteration ---- */
+  int opacity_kind;        /* 0 = the table (kappa_lo, alpha) above, independent of T;
+                              1 = kappa_lo[g] (T/T_ref)^p_T with the same alpha ("chi_g (T/T_0)^{3/2}");
+                              2 = ln kappa tabulated at the Nq+1 group EDGES on a uniform grid in ln T (lnk_edge below):
+                                  linear interpolation of ln kappa in ln T, end values outside the grid; the in-group
+                                  slope alpha_g follows from the two edge values of the group, Eq. 20.
+                                  kappa_lo and alpha are ignored (may be NULL); every edge must be finite and > 0.  */
+  double T_ref, p_T;       /* opacity_kind 1                                                                        */
+  int NT;                  /* opacity_kind 2: number of table temperatures (>= 1)                                   */
+  double lnT0, dlnT;       /*                 T_j = exp(lnT0 + j dlnT), j = 0..NT-1                                 */
+  const double *lnk_edge;  /*                 [Nq+1][NT] HOST, copied: ln of the specific opacity at edge e, temperature j */
 } mgrhd_opacity_model;
 
 /* Cell state, structure of arrays, float64, cell index fastest.  In mgrhd_source_update all
  * pointers are DEVICE pointers owned by the caller; mom, Egas, Erad, Frad are updated in
- * place, rho and kappa_scale are read only.  Arrays must not alias one another. */
+ * place, rho, kappa_scale and Srad are read only.  Arrays must not alias one another. */
 typedef struct {
   const double *rho;         /* [n]      gas density                                           */
   double *mom[3];            /* [n] each rho v                                                 */
@@ -72,6 +86,10 @@ typedef struct {
   double *Erad;              /* [Nq][n]  group radiation energy density E_g                    */
   double *Frad[3];           /* [Nq][n]  each: group radiation flux F_g^i                      */
   const double *kappa_scale; /* [n] per-cell multiplier on kappa_lo, or NULL (= 1)             */
+  const double *Srad;        /* [Nq][n]  optional source term S_g of Eq. 41: energy density added to
+                                group g during this update (e.g. stellar sources), or NULL (= 0).  Read only.
+                                E_g^(t+1) = E_g^(t) + R_g + S_g, E_tot of Eq. 50 includes sum_g S_g,
+                                and E_gas + (c/c_hat) sum_g (E_g - S_g) is conserved to round-off.                  */
 } mgrhd_state;
 
 /* Per-call diagnostics, accumulated on the device since the last mgrhd_reset_stats(). */
@@ -93,6 +111,9 @@ typedef struct {
  *   group_edges [Nq+1] HOST: nu_{g-}, ascending, >= 0; the last may be +inf.
  *   1 <= Nq <= MGRHD_MAX_GROUPS.  The context copies everything it needs (tables go to
  *   constant memory at launch); it uses the CUDA device current at the time of the call.
+ * Which kernel runs: the fixed-slope spectrum with opacity_kind 0 or 1 takes the tuned kernel (L lanes
+ * per cell); the free-slope spectrum and opacity_kind 2 take the general kernel (one
+ * warp per cell, lane = group), which needs the values of neighbouring groups.
  * Returns MGRHD_OK and *out, or a negative error (and *out = NULL). */
 int mgrhd_init(mgrhd_ctx **out, const double *group_edges, int Nq,
                const mgrhd_units *units, const mgrhd_opacity_model *model);

@@ -34,12 +34,15 @@ class Units(ctypes.Structure):
 class OpacityModel(ctypes.Structure):
     _fields_ = [("kappa_lo", _dp), ("alpha", _dp), ("closure", ctypes.c_int), ("spectrum", ctypes.c_int),
                 ("newton_tol", ctypes.c_double), ("newton_maxit", ctypes.c_int), ("outer_maxit", ctypes.c_int),
-                ("outer_tol", ctypes.c_double), ("outer_stop", ctypes.c_int), ("outer_rel_tol", ctypes.c_double)]
+                ("outer_tol", ctypes.c_double), ("outer_stop", ctypes.c_int), ("outer_rel_tol", ctypes.c_double),
+                ("opacity_kind", ctypes.c_int), ("T_ref", ctypes.c_double), ("p_T", ctypes.c_double),
+                ("NT", ctypes.c_int), ("lnT0", ctypes.c_double), ("dlnT", ctypes.c_double), ("lnk_edge", _dp)]
 
 
 class State(ctypes.Structure):
     _fields_ = [("rho", ctypes.c_void_p), ("mom", ctypes.c_void_p * 3), ("Egas", ctypes.c_void_p),
-                ("Erad", ctypes.c_void_p), ("Frad", ctypes.c_void_p * 3), ("kappa_scale", ctypes.c_void_p)]
+                ("Erad", ctypes.c_void_p), ("Frad", ctypes.c_void_p * 3), ("kappa_scale", ctypes.c_void_p),
+                ("Srad", ctypes.c_void_p)]
 
 
 class Stats(ctypes.Structure):
@@ -125,6 +128,9 @@ def _state_struct(state: dict, Nq: int, n: int) -> State:
     s.Egas = _ptr(state["Egas"])
     s.Erad = _ptr(state["Erad"])
     s.kappa_scale = _ptr(state.get("kappa_scale"))
+    if state.get("Srad") is not None:
+        assert tuple(state["Srad"].shape) == (Nq, n), ("Srad", tuple(state["Srad"].shape))
+    s.Srad = _ptr(state.get("Srad"))
     row = 8 * n
     m0, f0 = _ptr(state["mom"]), _ptr(state["Frad"])
     for k in range(3):
@@ -138,17 +144,24 @@ class Context:
 
     def __init__(self, edges, kappa_lo, alpha, *, a_rad=1.0, k_B=1.0, h_planck=1.0, mean_mass=1.0,
                  gamma=5.0 / 3.0, closure=0, spectrum=0, newton_tol=1e-11, newton_maxit=50, outer_maxit=50,
-                 outer_tol=1e-13, outer_stop=1, outer_rel_tol=1e-12):
+                 outer_tol=1e-13, outer_stop=1, outer_rel_tol=1e-12, opacity_kind=0, T_ref=1.0, p_T=0.0,
+                 lnT0=0.0, dlnT=1.0, lnk_edge=None):
         L = load_library()
         e = np.ascontiguousarray(edges, dtype=np.float64)
-        k = np.ascontiguousarray(kappa_lo, dtype=np.float64)
-        a = np.ascontiguousarray(alpha, dtype=np.float64)
-        self.Nq = int(k.shape[0])
-        if e.shape[0] != self.Nq + 1 or a.shape[0] != self.Nq:
-            raise MgrhdError("edges must have Nq+1 entries and alpha Nq")
+        self.Nq = int(e.shape[0]) - 1
+        k = None if kappa_lo is None else np.ascontiguousarray(kappa_lo, dtype=np.float64)
+        a = None if alpha is None else np.ascontiguousarray(alpha, dtype=np.float64)
+        if (k is not None and k.shape[0] != self.Nq) or (a is not None and a.shape[0] != self.Nq):
+            raise MgrhdError("edges must have Nq+1 entries and kappa_lo, alpha Nq")
+        t = None if lnk_edge is None else np.ascontiguousarray(lnk_edge, dtype=np.float64)
+        if t is not None and (t.ndim != 2 or t.shape[0] != self.Nq + 1):
+            raise MgrhdError("lnk_edge must be [Nq+1, NT]")
         u = Units(a_rad, k_B, h_planck, mean_mass, gamma)
-        m = OpacityModel(k.ctypes.data_as(_dp), a.ctypes.data_as(_dp), closure, spectrum, newton_tol,
-                         newton_maxit, outer_maxit, outer_tol, outer_stop, outer_rel_tol)
+        null = ctypes.cast(None, _dp)
+        m = OpacityModel(null if k is None else k.ctypes.data_as(_dp), null if a is None else a.ctypes.data_as(_dp),
+                         closure, spectrum, newton_tol, newton_maxit, outer_maxit, outer_tol, outer_stop, outer_rel_tol,
+                         opacity_kind, T_ref, p_T, 0 if t is None else t.shape[1], lnT0, dlnT,
+                         null if t is None else t.ctypes.data_as(_dp))
         h = ctypes.c_void_p()
         _check(L.mgrhd_init(ctypes.byref(h), e.ctypes.data_as(_dp), self.Nq, ctypes.byref(u), ctypes.byref(m)),
                "mgrhd_init")
@@ -156,11 +169,16 @@ class Context:
         self._L = L
 
     @classmethod
-    def from_workload(cls, wl) -> "Context":
-        return cls(wl.edges, wl.kappa_lo, wl.alpha, a_rad=wl.a_rad, k_B=wl.k_B, h_planck=wl.h_planck,
-                   mean_mass=wl.mean_mass, gamma=wl.gamma, closure=wl.closure, newton_tol=wl.newton_tol,
-                   newton_maxit=wl.newton_maxit, outer_maxit=wl.outer_maxit, outer_tol=wl.outer_tol,
-                   outer_stop=wl.outer_stop, outer_rel_tol=wl.outer_rel_tol)
+    def from_workload(cls, wl, **kw) -> "Context":
+        args = dict(a_rad=wl.a_rad, k_B=wl.k_B, h_planck=wl.h_planck,
+                    mean_mass=wl.mean_mass, gamma=wl.gamma, closure=wl.closure, newton_tol=wl.newton_tol,
+                    newton_maxit=wl.newton_maxit, outer_maxit=wl.outer_maxit, outer_tol=wl.outer_tol,
+                    outer_stop=wl.outer_stop, outer_rel_tol=wl.outer_rel_tol)
+        for key in ("spectrum", "opacity_kind", "T_ref", "p_T", "lnT0", "dlnT", "lnk_edge"):   # optional model fields
+            if hasattr(wl, key):
+                args[key] = getattr(wl, key)
+        args.update(kw)
+        return cls(wl.edges, wl.kappa_lo, wl.alpha, **args)
 
     def source_update(self, state: dict, dt: float, c: float, c_hat: float, stream=None) -> None:
         """mgrhd_source_update on DEVICE tensors, in place, stream-ordered (default: torch's current stream)."""

@@ -11,7 +11,7 @@
 #include <mutex>
 #include <new>
 
-#include "mgrhd_kernels.cuh"
+#include "mgrhd_general.cuh"
 
 using namespace mgrhd;
 
@@ -146,6 +146,9 @@ constexpr long long kSlabBytes = 96ll << 20;    // target bytes per slab
 
 struct mgrhd_ctx {
   Params P;
+  GenParams G;
+  int general;                        // 1: the general kernel (free-slope spectrum, opacity_kind 2) runs
+  double* d_lnk;                      // opacity_kind 2: device copy of the edge table
   int device;
   int sm_count;
   unsigned long long* d_stats;
@@ -165,24 +168,24 @@ struct mgrhd_ctx {
 // One instantiation per (lanes per cell L, steps per lane NQL, CTA size): chosen so that the
 // [slot][step][thread] state fits in shared memory (SL_COUNT * NQL * THREADS * 8 bytes <= 227 KB)
 // with as many threads per SM as the register file allows.
-template <int L, int NQL, int THREADS>
+template <int L, int NQL, int THREADS, bool KT>
 struct Inst {
   static constexpr size_t kSmem = (size_t)SL_COUNT * NQL * THREADS * sizeof(double);
   static cudaError_t configure(int* blocks_per_sm) {
-    cudaError_t e = cudaFuncSetAttribute(source_update_kernel<L, NQL, THREADS, false>,
+    cudaError_t e = cudaFuncSetAttribute(source_update_kernel<L, NQL, THREADS, KT, false>,
                                          cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem);
     if (e == cudaSuccess)
-      e = cudaFuncSetAttribute(source_update_kernel<L, NQL, THREADS, true>,
+      e = cudaFuncSetAttribute(source_update_kernel<L, NQL, THREADS, KT, true>,
                                cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem);
     if (e == cudaSuccess)
-      e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, source_update_kernel<L, NQL, THREADS, false>,
+      e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, source_update_kernel<L, NQL, THREADS, KT, false>,
                                                         THREADS, kSmem);
     return e;
   }
   static void launch(bool count, unsigned blocks, cudaStream_t st, const Params& P, const StatePtrs& S,
                      unsigned long long* stats, double* scratch) {
-    if (count) source_update_kernel<L, NQL, THREADS, true><<<blocks, THREADS, kSmem, st>>>(P, S, stats, scratch);
-    else source_update_kernel<L, NQL, THREADS, false><<<blocks, THREADS, kSmem, st>>>(P, S, stats, scratch);
+    if (count) source_update_kernel<L, NQL, THREADS, KT, true><<<blocks, THREADS, kSmem, st>>>(P, S, stats, scratch);
+    else source_update_kernel<L, NQL, THREADS, KT, false><<<blocks, THREADS, kSmem, st>>>(P, S, stats, scratch);
   }
 };
 
@@ -200,7 +203,10 @@ struct Inst {
 // Fills ctx->cfg_* for ctx->P.Nq (called once by mgrhd_init).
 static cudaError_t configure_ctx(mgrhd_ctx* ctx) {
   cudaError_t e = cudaSuccess;
-#define MGRHD_CFG(LL, Q, T) e = Inst<LL, Q, T>::configure(&ctx->cfg_bps); ctx->cfg_l = LL; ctx->cfg_nq = Q; ctx->cfg_threads = T
+#define MGRHD_CFG(LL, Q, T)                                                                                 \
+  e = kt ? Inst<LL, Q, T, true>::configure(&ctx->cfg_bps) : Inst<LL, Q, T, false>::configure(&ctx->cfg_bps); \
+  ctx->cfg_l = LL; ctx->cfg_nq = Q; ctx->cfg_threads = T
+  const bool kt = ctx->G.opacity_kind == 1;
   MGRHD_DISPATCH(ctx->P.Nq, MGRHD_CFG);
 #undef MGRHD_CFG
   if (e == cudaSuccess && ctx->cfg_bps < 1) e = cudaErrorLaunchOutOfResources;
@@ -219,17 +225,31 @@ const char* mgrhd_last_error(void) { return g_err; }
 int mgrhd_init(mgrhd_ctx** out, const double* edges, int Nq, const mgrhd_units* u,
                const mgrhd_opacity_model* m) {
   if (out) *out = nullptr;
-  if (!out || !edges || !u || !m || !m->kappa_lo || !m->alpha) return MGRHD_ERR_ARG;
+  if (!out || !edges || !u || !m) return MGRHD_ERR_ARG;
+  if (m->opacity_kind < 0 || m->opacity_kind > 2) return MGRHD_ERR_ARG;
+  const bool tab = m->opacity_kind == 2;
+  if (!tab && (!m->kappa_lo || !m->alpha)) return MGRHD_ERR_ARG;
+  if (tab && (!m->lnk_edge || m->NT < 1)) return MGRHD_ERR_ARG;
   if (Nq < 1 || Nq > MGRHD_MAX_GROUPS) return MGRHD_ERR_ARG;
-  if (m->closure < 0 || m->closure > 1 || m->spectrum != 0) return MGRHD_ERR_ARG;
+  if (m->closure < 0 || m->closure > 1 || m->spectrum < 0 || m->spectrum > 1) return MGRHD_ERR_ARG;
   if (m->outer_stop < 0 || m->outer_stop > 1 || m->newton_maxit < 1 || m->outer_maxit < 1)
     return MGRHD_ERR_ARG;
   if (!(u->a_rad > 0) || !(u->k_B > 0) || !(u->h_planck > 0) || !(u->mean_mass > 0) ||
       !(u->gamma > 1) || !(m->newton_tol > 0) || !(m->outer_tol > 0))
     return MGRHD_ERR_RANGE;
+  if (m->opacity_kind == 1 && (!(m->T_ref > 0) || !std::isfinite(m->T_ref) || !std::isfinite(m->p_T))) return MGRHD_ERR_RANGE;
+  if (tab && m->NT > 1 && (!(m->dlnT > 0) || !std::isfinite(m->dlnT) || !std::isfinite(m->lnT0))) return MGRHD_ERR_RANGE;
+  if (tab)
+    for (long long i = 0; i < (long long)(Nq + 1) * m->NT; ++i)
+      if (!std::isfinite(m->lnk_edge[i])) return MGRHD_ERR_RANGE;
   for (int g = 0; g < Nq; ++g) {
     if (!(edges[g] >= 0.0) || !(edges[g + 1] > edges[g])) return MGRHD_ERR_EDGES;
-    if (m->alpha[g] != 0.0 && (edges[g] == 0.0 || std::isinf(edges[g + 1]))) return MGRHD_ERR_ALPHA;
+    const bool open_group = edges[g] == 0.0 || std::isinf(edges[g + 1]);
+    if (tab) {
+      if (open_group) return MGRHD_ERR_ALPHA;       // Eq. 20 needs both edge values of every group
+      continue;
+    }
+    if (m->alpha[g] != 0.0 && open_group) return MGRHD_ERR_ALPHA;
     // kappa = 0 makes Eq. 42 singular (E_g = ... /chi_E): rejected, as are inf/NaN
     if (!std::isfinite(m->alpha[g]) || !(m->kappa_lo[g] > 0.0) || !std::isfinite(m->kappa_lo[g])) return MGRHD_ERR_RANGE;
   }
@@ -249,8 +269,25 @@ int mgrhd_init(mgrhd_ctx** out, const double* edges, int Nq, const mgrhd_units* 
   P.h_over_k = u->h_planck / u->k_B;
   P.cv_over_rho = u->k_B / ((u->gamma - 1.0) * u->mean_mass);
   for (int g = 0; g <= Nq; ++g) P.nu[g] = edges[g];
+  P.inv_T_ref = m->opacity_kind == 1 ? 1.0 / m->T_ref : 1.0;
+  P.p_T = m->opacity_kind == 1 ? m->p_T : 0.0;
+  GenParams& G = ctx->G;
+  G.spectrum = m->spectrum;
+  G.opacity_kind = m->opacity_kind;
+  G.NT = tab ? m->NT : 0;
+  G.lnT0 = tab ? m->lnT0 : 0.0;
+  G.inv_dlnT = tab && m->NT > 1 ? 1.0 / m->dlnT : 0.0;
   for (int g = 0; g < Nq; ++g) {
-    const double a = m->alpha[g], k = m->kappa_lo[g];
+    const bool open_group = edges[g] == 0.0 || std::isinf(edges[g + 1]);
+    G.lnr[g] = open_group ? 0.0 : std::log(edges[g + 1] / edges[g]);
+    G.width[g] = edges[g + 1] - edges[g];
+    G.inv_lnnb[g] = 0.0;
+    if (g + 1 < Nq && edges[g] > 0.0 && std::isfinite(edges[g + 2]))     // Eq. A1 between groups g and g + 1
+      G.inv_lnnb[g] = 1.0 / std::log(std::sqrt(edges[g + 2] * edges[g + 1]) / std::sqrt(edges[g + 1] * edges[g]));
+  }
+  ctx->general = (m->spectrum == 1 || tab) ? 1 : 0;
+  for (int g = 0; g < Nq; ++g) {
+    const double a = tab ? 0.0 : m->alpha[g], k = tab ? 1.0 : m->kappa_lo[g];
     P.alpha[g] = a;
     P.k_lo[g] = k;
     if (a == 0.0) {                       // piecewise constant, Eq. 17
@@ -270,12 +307,19 @@ int mgrhd_init(mgrhd_ctx** out, const double* edges, int Nq, const mgrhd_units* 
   if (e == cudaSuccess) e = upload_tables_for_current_device();
   if (e == cudaSuccess) e = configure_ctx(ctx);
   if (e == cudaSuccess) e = cudaMalloc(&ctx->scratch, scratch_bytes(ctx));
+  if (e == cudaSuccess && tab) {
+    const size_t bytes = (size_t)(Nq + 1) * m->NT * sizeof(double);
+    e = cudaMalloc(&ctx->d_lnk, bytes);
+    if (e == cudaSuccess) e = cudaMemcpy(ctx->d_lnk, m->lnk_edge, bytes, cudaMemcpyHostToDevice);
+    G.lnk_edge = ctx->d_lnk;
+  }
   if (e == cudaSuccess) e = cudaMalloc(&ctx->d_stats, kStatCount * sizeof(unsigned long long));
   if (e == cudaSuccess) e = cudaMemset(ctx->d_stats, 0, kStatCount * sizeof(unsigned long long));
   if (e != cudaSuccess) {
     cuda_ok(e, "mgrhd_init");
     if (ctx->d_stats) cudaFree(ctx->d_stats);
     if (ctx->scratch) cudaFree(ctx->scratch);
+    if (ctx->d_lnk) cudaFree(ctx->d_lnk);
     delete ctx;
     return MGRHD_ERR_CUDA;
   }
@@ -306,7 +350,22 @@ static int launch_update(mgrhd_ctx* ctx, const StatePtrs& S, long long n, long l
   if (blocks > want) blocks = want;
   const bool count = ctx->count_flops != 0;
   CU(cudaMemsetAsync(scratch, 0, kScratchHead * sizeof(double), st));   // work counter of the chunk scheduler
-#define MGRHD_GO(LL, Q, T) Inst<LL, Q, T>::launch(count, (unsigned)blocks, st, P, S, ctx->d_stats, scratch)
+  if (ctx->general) {
+    // one warp per cell, 8 warps per CTA, persistent grid (8 CTAs per SM at most)
+    long long gb = (n + 7) / 8;
+    const long long cap = (long long)ctx->sm_count * 8;
+    if (gb > cap) gb = cap;
+    if (P.Nq <= 32) source_update_general_kernel<1><<<(unsigned)gb, 256, 0, st>>>(P, ctx->G, S, ctx->d_stats);
+    else source_update_general_kernel<2><<<(unsigned)gb, 256, 0, st>>>(P, ctx->G, S, ctx->d_stats);
+    ctx->launches++;
+    ctx->last_stream = st;
+    CU(cudaGetLastError());
+    return MGRHD_OK;
+  }
+  const bool kt = ctx->G.opacity_kind == 1;
+#define MGRHD_GO(LL, Q, T)                                                                        \
+  if (kt) Inst<LL, Q, T, true>::launch(count, (unsigned)blocks, st, P, S, ctx->d_stats, scratch); \
+  else Inst<LL, Q, T, false>::launch(count, (unsigned)blocks, st, P, S, ctx->d_stats, scratch)
   MGRHD_DISPATCH(P.Nq, MGRHD_GO);
 #undef MGRHD_GO
   ctx->launches++;
@@ -322,6 +381,7 @@ static StatePtrs to_ptrs(const mgrhd_state* s) {
   S.Egas = s->Egas;
   S.Erad = s->Erad;
   S.kappa_scale = s->kappa_scale;
+  S.Srad = s->Srad;
   return S;
 }
 
@@ -356,7 +416,7 @@ int mgrhd_source_update_host(mgrhd_ctx* ctx, const mgrhd_state* s, long long n, 
   if (rc != MGRHD_OK) return rc;
   if (n == 0) return MGRHD_OK;
   const int Nq = ctx->P.Nq;
-  const long long per_cell = 6 + 4ll * Nq;     // rho, mom[3], Egas, kappa_scale, Erad, Frad[3]
+  const long long per_cell = 6 + 5ll * Nq;     // rho, mom[3], Egas, kappa_scale, Erad, Frad[3], Srad
   if (!ctx->slab[0]) {
     long long sc = kSlabBytes / (8 * per_cell);
     sc = (sc / 1024) * 1024;
@@ -385,6 +445,8 @@ int mgrhd_source_update_host(mgrhd_ctx* ctx, const mgrhd_state* s, long long n, 
     S.kappa_scale = s->kappa_scale ? d_ks : nullptr;
     S.Erad = q; q += sc * Nq;
     for (int i = 0; i < 3; ++i) { S.Frad[i] = q; q += sc * Nq; }
+    double* d_S = q; q += sc * Nq;
+    S.Srad = s->Srad ? d_S : nullptr;
     // host -> device
     CU(cudaMemcpyAsync((void*)S.rho, s->rho + lo, w, cudaMemcpyHostToDevice, st));
     for (int i = 0; i < 3; ++i) CU(cudaMemcpyAsync(S.mom[i], s->mom[i] + lo, w, cudaMemcpyHostToDevice, st));
@@ -393,6 +455,7 @@ int mgrhd_source_update_host(mgrhd_ctx* ctx, const mgrhd_state* s, long long n, 
     CU(cudaMemcpy2DAsync(S.Erad, pitch_d, s->Erad + lo, pitch_h, w, Nq, cudaMemcpyHostToDevice, st));
     for (int i = 0; i < 3; ++i)
       CU(cudaMemcpy2DAsync(S.Frad[i], pitch_d, s->Frad[i] + lo, pitch_h, w, Nq, cudaMemcpyHostToDevice, st));
+    if (s->Srad) CU(cudaMemcpy2DAsync(d_S, pitch_d, s->Srad + lo, pitch_h, w, Nq, cudaMemcpyHostToDevice, st));
     // update
     rc = launch_update(ctx, S, m, sc, dt, c, chat, st, ctx->slab_scratch[j]);
     if (rc != MGRHD_OK) return rc;
@@ -495,6 +558,7 @@ void mgrhd_free(mgrhd_ctx* ctx) {
   }
   if (ctx->d_stats) cudaFree(ctx->d_stats);
   if (ctx->scratch) cudaFree(ctx->scratch);
+  if (ctx->d_lnk) cudaFree(ctx->d_lnk);
   delete ctx;
 }
 

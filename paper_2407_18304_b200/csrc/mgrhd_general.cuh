@@ -1,0 +1,394 @@
+// mgrhd_general.cuh -- the general kernel of the implicit source update: one WARP
+// per cell, lane j owns the GPL consecutive groups g = j*GPL .. j*GPL + GPL-1, everything in registers.
+//
+// It exists for the model options whose group evaluation needs the values of NEIGHBOURING groups and
+// therefore does not fit the tuned kernel's lanes-per-cell state machine (mgrhd_kernels.cuh):
+//   * the PPL free-slope spectrum fit of Appendix A (Eq. A1-A2): alpha_B,g and
+//     alpha_E,g from the group integrals of the two neighbours, refitted at every Newton evaluation,
+//     chi_B != chi_E from Eq. 30;
+//   * opacity_kind 2: opacities tabulated at the group EDGES in ln T, alpha_g from the two edge values
+//     of the group (Eq. 20) at every trial temperature.
+// With lane = group a neighbour is one shuffle away and the sums of Eq. 48-52 are full-warp butterflies.
+// It also runs every other option (opacity_kind 0/1, S_g), which the tests use to cross-check the two
+// kernels.  The iteration (iterates, stopping tests, guards, readings S8-S10, S19-S21 of DESIGN.md) is the
+// same as the tuned kernel's; the Planck edge functions and the closure are the same device functions.
+//
+// Cost: every lane of a warp evaluates a different edge, so all three branches of the edge functions run
+// in every evaluation, and a cell's 4 Nq + 5 loads touch 4 Nq + 5 different sectors (cell index is the
+// fastest in the state): a feature path, measured separately, not the benchmark path.
+//
+// Product code; shares nothing with oracle/.
+#pragma once
+#include "mgrhd_kernels.cuh"
+
+namespace mgrhd {
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) v += __shfl_xor_sync(0xffffffffu, v, off);
+  return v;
+}
+
+// [ (r^q - 1)/q ] of Eq. 30, ln r at q ln r = 0.
+__device__ __forceinline__ double eq30_bracket(double q, double lnr) {
+  const double z = q * lnr;
+  return z == 0.0 ? lnr : expm1(z) / q;
+}
+
+// minmod of Eq. A2.
+__device__ __forceinline__ double minmod(double a, double b) {
+  if (a * b <= 0.0) return 0.0;
+  return fabs(a) < fabs(b) ? a : b;
+}
+
+// Eq. A1-A2 for the lane's groups: Q[k] group integrals (all lanes call; converged warp).
+//   alpha_Q,g = minmod(s_{g-1/2}, s_{g+1/2}), s_{g+1/2} = ln(Qbar_{g+1}/Qbar_g)/ln(nubar_{g+1}/nubar_g);
+//   edge groups, and groups next to a non-positive Q or an open group, get -1 (reading S21).
+template <int GPL>
+__device__ __forceinline__ void free_slopes(const GenParams& G, int Nq, int lane, const double (&Q)[GPL],
+                                            double (&aQ)[GPL]) {
+  const unsigned FULL = 0xffffffffu;
+  double qb[GPL], s_up[GPL];
+  bool ok_up[GPL];
+#pragma unroll
+  for (int k = 0; k < GPL; ++k) {
+    const int g = lane * GPL + k;
+    qb[k] = g < Nq ? Q[k] / G.width[g < Nq ? g : 0] : 0.0;
+  }
+  const double qb_right = __shfl_down_sync(FULL, qb[0], 1);           // first group of the lane to the right
+#pragma unroll
+  for (int k = 0; k < GPL; ++k) {
+    const int g = lane * GPL + k;
+    const double qn = k + 1 < GPL ? qb[k + 1 < GPL ? k + 1 : 0] : qb_right;
+    const double il = g + 1 < Nq ? G.inv_lnnb[g] : 0.0;
+    ok_up[k] = g + 1 < Nq && qb[k] > 0.0 && qn > 0.0 && il != 0.0 && !(lane == 31 && k == GPL - 1);
+    s_up[k] = ok_up[k] ? log(qn / qb[k]) * il : 0.0;
+  }
+  const double s_left = __shfl_up_sync(FULL, s_up[GPL - 1], 1);       // s_{g-1/2} of the lane's first group
+  const int ok_left = __shfl_up_sync(FULL, (int)ok_up[GPL - 1], 1);
+#pragma unroll
+  for (int k = 0; k < GPL; ++k) {
+    const int g = lane * GPL + k;
+    const double sd = k > 0 ? s_up[k > 0 ? k - 1 : 0] : s_left;
+    const bool okd = k > 0 ? ok_up[k > 0 ? k - 1 : 0] : (lane > 0 && ok_left != 0);
+    const bool interior = g >= 1 && g + 1 < Nq;
+    aQ[k] = interior && okd && ok_up[k] ? minmod(sd, s_up[k]) : -1.0;
+  }
+}
+
+enum GenStat : int { GS_EVALS = 0, GS_TRIPS, GS_GUARD, GS_DEN, GS_COUNT };
+
+// GPL: groups per lane (1: Nq <= 32, 2: Nq <= 64).  256 threads = 8 warps = 8 cells in flight per CTA.
+template <int GPL>
+__global__ void __launch_bounds__(256)
+source_update_general_kernel(const __grid_constant__ Params P, const __grid_constant__ GenParams G,
+                             const __grid_constant__ StatePtrs S, unsigned long long* __restrict__ stats) {
+  __shared__ unsigned int s_hist[2 * MGRHD_HIST];
+  __shared__ unsigned int s_cnt[GS_COUNT];
+  for (int t = threadIdx.x; t < 2 * MGRHD_HIST; t += blockDim.x) s_hist[t] = 0u;
+  if (threadIdx.x < GS_COUNT) s_cnt[threadIdx.x] = 0u;
+  __syncthreads();
+
+  const unsigned FULL = 0xffffffffu;
+  const int lane = threadIdx.x & 31;
+  const int Nq = P.Nq;
+  const long long n = P.ncells, stride = P.stride;
+  const double dt = P.dt, c = P.c, chat = P.c_hat;
+  const double c_over_chat = c / chat, cdt = chat * dt, icc = 1.0 / (c * chat);
+  const double NaN = __longlong_as_double(0x7ff8000000000000ll);
+  const long long nwarps = ((long long)gridDim.x * blockDim.x) >> 5;
+  const long long warp0 = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+
+  // per-group constants of the lane's groups
+  int gi[GPL];
+  bool vg[GPL];
+  double nu_hi[GPL], lnr[GPL], k_lo[GPL], k_hi[GPL], al_tab[GPL];
+#pragma unroll
+  for (int k = 0; k < GPL; ++k) {
+    const int g = lane * GPL + k;
+    vg[k] = g < Nq;
+    gi[k] = vg[k] ? g : 0;
+    nu_hi[k] = P.nu[gi[k] + 1];
+    lnr[k] = G.lnr[gi[k]];
+    k_lo[k] = P.k_lo[gi[k]];
+    k_hi[k] = P.k_hi[gi[k]];
+    al_tab[k] = P.alpha[gi[k]];
+  }
+
+  for (long long cell = warp0; cell < n; cell += nwarps) {
+    // ---- a0: load (the post-explicit state U^(t)) --------------------------------------
+    const double rho = S.rho[cell];
+    const double ks = S.kappa_scale ? S.kappa_scale[cell] : 1.0;
+    const double momt0 = S.mom[0][cell], momt1 = S.mom[1][cell], momt2 = S.mom[2][cell];
+    const double Egas_t = S.Egas[cell];
+    const double chis = rho * ks, inv_rho = 1.0 / rho;
+    const double Cv = rho * P.cv_over_rho;
+    double Et[GPL], Sg[GPL], R[GPL], Ft0[GPL], Ft1[GPL], Ft2[GPL], Fk0[GPL], Fk1[GPL], Fk2[GPL];
+    double Fn0[GPL], Fn1[GPL], Fn2[GPL], Enew[GPL];
+    double sumEtS = 0.0;
+#pragma unroll
+    for (int k = 0; k < GPL; ++k) {
+      const long long o = (long long)gi[k] * stride + cell;
+      Et[k] = vg[k] ? S.Erad[o] : 0.0;
+      Sg[k] = vg[k] && S.Srad ? S.Srad[o] : 0.0;
+      Ft0[k] = vg[k] ? S.Frad[0][o] : 0.0; Ft1[k] = vg[k] ? S.Frad[1][o] : 0.0; Ft2[k] = vg[k] ? S.Frad[2][o] : 0.0;
+      Fk0[k] = Ft0[k]; Fk1[k] = Ft1[k]; Fk2[k] = Ft2[k];
+      Fn0[k] = Ft0[k]; Fn1[k] = Ft1[k]; Fn2[k] = Ft2[k];
+      R[k] = 0.0;
+      Enew[k] = Et[k];
+      sumEtS += Et[k] + Sg[k];
+    }
+    const double Etot = Egas_t + (chat / c) * warp_sum(sumEtS);        // Eq. 50 as printed
+    double momk0 = momt0, momk1 = momt1, momk2 = momt2, momn0 = momt0, momn1 = momt1, momn2 = momt2;
+    double Egs = Egas_t, Egas_new = Egas_t;
+    int evals = 0, trips = 0;
+    // group quantities of the last evaluation (used by Eq. 51 and the outer test)
+    double alpha[GPL], chiE[GPL], chiF[GPL], AG[GPL], W[GPL];
+
+    for (int kk = 0; kk < P.outer_maxit; ++kk) {
+      // ---- O1: lagged velocity and fluxes -------------------------------------------
+      const double v0 = momk0 * inv_rho, v1 = momk1 * inv_rho, v2 = momk2 * inv_rho;
+      const double Ekin = (momk0 * momk0 + momk1 * momk1 + momk2 * momk2) * (0.5 * inv_rho);
+      double vF[GPL];
+#pragma unroll
+      for (int k = 0; k < GPL; ++k) vF[k] = fma(v0, Fk0[k], fma(v1, Fk1[k], v2 * Fk2[k]));
+      if (!((Egs - Ekin) / Cv > 0.0)) {                                // invalid state: stop here (S9)
+        if (lane == 0) atomicAdd(&stats[kStatTNonPos], 1ull);
+        break;
+      }
+      // ---- inner Newton-Raphson iteration on x = (E_gas, R_1..R_Nq) (Eq. 41-50) ---------------------
+      for (int it = 0;; ++it) {
+        const double T = (Egs - Ekin) / Cv;
+        const double T2 = T * T, aT4 = P.a_rad * T2 * T2;
+        const double beta = P.h_over_k / T;
+        // a1: edge functions at the lane's upper edges; the lower edge comes from the left, edge 0 from an
+        // evaluation of its own (lane 0)
+        double hy[GPL], hx[GPL], ly[GPL], lx[GPL];
+        bool hs[GPL], ls[GPL];
+        int fl;
+#pragma unroll
+        for (int k = 0; k < GPL; ++k)
+          planck_edge_w(vg[k] ? nu_hi[k] * beta : NaN, 0, hy[k], hx[k], hs[k], fl);
+        double e0y, e0x;
+        bool e0s;
+        planck_edge_w(lane == 0 ? P.nu[0] * beta : NaN, 0, e0y, e0x, e0s, fl);
+        {
+          const double uy = __shfl_up_sync(FULL, hy[GPL - 1], 1), ux = __shfl_up_sync(FULL, hx[GPL - 1], 1);
+          const int us = __shfl_up_sync(FULL, (int)hs[GPL - 1], 1);
+#pragma unroll
+          for (int k = 0; k < GPL; ++k) {
+            ly[k] = k > 0 ? hy[k > 0 ? k - 1 : 0] : (lane == 0 ? e0y : uy);
+            lx[k] = k > 0 ? hx[k > 0 ? k - 1 : 0] : (lane == 0 ? e0x : ux);
+            ls[k] = k > 0 ? hs[k > 0 ? k - 1 : 0] : (lane == 0 ? e0s : us != 0);
+          }
+        }
+        // a2: group Planck integrals per unit a_R T^4 (Eq. 11): no cancellation in the Wien tail
+        double dY[GPL], dX[GPL], Bt[GPL];
+#pragma unroll
+        for (int k = 0; k < GPL; ++k) {
+          dY[k] = hs[k] ? hy[k] - ly[k] : (ls[k] ? (1.0 - ly[k]) - hy[k] : ly[k] - hy[k]);
+          dX[k] = hx[k] - lx[k];
+          Bt[k] = vg[k] ? aT4 * dY[k] : 0.0;
+        }
+        // a3: opacities at the group edges at this trial temperature (Eq. 19, 20)
+        double chi_lo[GPL], chi_hi[GPL];
+        if (G.opacity_kind == 2) {
+          const double lnT = log(T);
+          double u = (lnT - G.lnT0) * G.inv_dlnT;
+          if (!(u > 0.0)) u = 0.0;
+          if (u > (double)(G.NT - 1)) u = (double)(G.NT - 1);
+          int j = (int)u;
+          if (j > G.NT - 2) j = G.NT - 2;
+          if (j < 0) j = 0;
+          const double w = G.NT > 1 ? u - (double)j : 0.0;
+          auto edge_chi = [&](int e) {
+            const double* row = G.lnk_edge + (long long)e * G.NT;
+            const double lnk = G.NT > 1 ? (1.0 - w) * row[j] + w * row[j + 1] : row[0];
+            return chis * exp(lnk);
+          };
+#pragma unroll
+          for (int k = 0; k < GPL; ++k) chi_hi[k] = edge_chi(gi[k] + 1);
+          const double c0 = edge_chi(0);
+          const double cu = __shfl_up_sync(FULL, chi_hi[GPL - 1], 1);
+#pragma unroll
+          for (int k = 0; k < GPL; ++k) {
+            chi_lo[k] = k > 0 ? chi_hi[k > 0 ? k - 1 : 0] : (lane == 0 ? c0 : cu);
+            alpha[k] = log(chi_hi[k] / chi_lo[k]) / lnr[k];                        // Eq. 20
+          }
+        } else {
+          const double f = G.opacity_kind == 1 ? pow(T * P.inv_T_ref, P.p_T) : 1.0;
+#pragma unroll
+          for (int k = 0; k < GPL; ++k) {
+            alpha[k] = al_tab[k];
+            chi_lo[k] = chis * k_lo[k] * f;
+            chi_hi[k] = chis * k_hi[k] * f;                                        // Eq. 19 at nu_g+
+          }
+        }
+        // spectrum slopes alpha_B,g, alpha_E,g (fixed: -1; free: Appendix A, refitted from B_g at
+        // this T and from the current iterate E_g^(t) + R_g + S_g, reading S20) and the means of Eq. 30
+        double aB[GPL], aE[GPL], chiB[GPL];
+#pragma unroll
+        for (int k = 0; k < GPL; ++k) { aB[k] = -1.0; aE[k] = -1.0; }
+        if (G.spectrum == 1) {
+          double Ecur[GPL];
+#pragma unroll
+          for (int k = 0; k < GPL; ++k) Ecur[k] = Et[k] + R[k] + Sg[k];
+          free_slopes<GPL>(G, Nq, lane, Bt, aB);
+          free_slopes<GPL>(G, Nq, lane, Ecur, aE);
+        }
+        double sumR = 0.0, sumAbsFR = 0.0, SFRq = 0.0, SJq = 0.0, FR[GPL], qg[GPL], jg0[GPL];
+        unsigned n_guard = 0, n_den = 0;
+#pragma unroll
+        for (int k = 0; k < GPL; ++k) {
+          if (alpha[k] == 0.0) {
+            chiB[k] = chi_lo[k];                                                   // PC, Eq. 17
+            chiE[k] = chi_lo[k];
+          } else {
+            chiB[k] = chi_lo[k] * eq30_bracket(alpha[k] + aB[k] + 1.0, lnr[k]) / eq30_bracket(aB[k] + 1.0, lnr[k]);
+            chiE[k] = chi_lo[k] * eq30_bracket(alpha[k] + aE[k] + 1.0, lnr[k]) / eq30_bracket(aE[k] + 1.0, lnr[k]);
+          }
+          // a2: Doppler boundary term Delta_g(nu chi_0 B_nu) per unit a_R T^4 (Eq. 22)
+          const double P3 = fma(chi_hi[k], hx[k], -chi_lo[k] * lx[k]);
+          const double fbd = fma(4.0, dY[k], -dX[k]);                              // 3 x denominator of Eq. 27
+          // a3: flux-mean opacity, Eq. 27, with the guards of reading S8
+          const bool guard = !(fbd >= 3e-280) || isinf(aT4 * fbd);
+          double cf = (fma(3.0 * chiB[k] + (1.0 + alpha[k]) * chiE[k], dY[k], -P3)) / (guard ? 1.0 : fbd);
+          if (guard) cf = chi_lo[k];
+          const bool denbad = !(fma(cdt, cf, 1.0) > 0.0);
+          if (denbad) cf = chiE[k];
+          if (vg[k] && evals == 0) { n_guard += guard ? 1u : 0u; n_den += denbad ? 1u : 0u; }
+          chiF[k] = cf;
+          // a4: work term, Eq. 42 solved for E_g, residuals of Eq. 41
+          W[k] = (1.0 + alpha[k]) * cf * vF[k] / c;
+          const double ratio = chiB[k] / chiE[k];
+          const double Eg = ratio * Bt[k] + W[k] / (c * chiE[k]) - R[k] / (cdt * chiE[k]);
+          FR[k] = vg[k] ? Eg - Et[k] - (R[k] + Sg[k]) : 0.0;
+          // a5: Jacobian, Eq. 44-47 (d(chi_B/chi_E)/dT = 0), q = -1/J_gg
+          qg[k] = 1.0 / (1.0 / (cdt * chiE[k]) + 1.0);
+          jg0[k] = ratio * (aT4 * fbd / T) / Cv;                                   // (4 Bt - Db)/T / C_v
+          AG[k] = aT4 * fma(chiB[k], dY[k], P3 * (-1.0 / 3.0));                    // chi_B Bt - D/3 (Eq. 51 source)
+          if (vg[k]) {
+            sumR += R[k];
+            sumAbsFR += fabs(FR[k]);
+            SFRq += FR[k] * qg[k];
+            SJq += jg0[k] * qg[k];
+          }
+        }
+        sumR = warp_sum(sumR); sumAbsFR = warp_sum(sumAbsFR); SFRq = warp_sum(SFRq); SJq = warp_sum(SJq);
+        if (evals == 0) {
+          const unsigned ng = __reduce_add_sync(FULL, n_guard), nd = __reduce_add_sync(FULL, n_den);
+          if (lane == 0 && ng) atomicAdd(&s_cnt[GS_GUARD], ng);
+          if (lane == 0 && nd) atomicAdd(&s_cnt[GS_DEN], nd);
+        }
+        const double FG = Egs - Egas_t + c_over_chat * sumR;
+        evals++;
+        // Eq. 49
+        if (fabs(FG) / Etot < P.newton_tol && c_over_chat * sumAbsFR / Etot < P.newton_tol) break;
+        if (it >= P.newton_maxit) {
+          if (lane == 0) atomicAdd(&stats[kStatNewtonUnconv], 1ull);
+          break;
+        }
+        // Newton step: eliminate the gas row of the arrowhead Jacobian (Eq. 48)
+        const double dx0 = (-FG - c_over_chat * SFRq) / fma(c_over_chat, SJq, 1.0);
+        double lam = 1.0;
+        for (int h = 0; h < 10 && !((Egs + lam * dx0 - Ekin) / Cv > 0.0); ++h) {   // S9
+          lam *= 0.5;
+          if (lane == 0) atomicAdd(&stats[kStatTNonPos], 1ull);
+        }
+        Egs += lam * dx0;
+#pragma unroll
+        for (int k = 0; k < GPL; ++k) R[k] += lam * (FR[k] + jg0[k] * dx0) * qg[k];
+      }
+
+      // ---- a6: energy commit ---------------------------------------------------------
+      double sR = 0.0, sAbsR = 0.0;
+#pragma unroll
+      for (int k = 0; k < GPL; ++k) {
+        Enew[k] = Et[k] + R[k] + Sg[k];
+        if (vg[k]) { sR += R[k]; sAbsR += fabs(R[k]); }
+      }
+      sR = warp_sum(sR); sAbsR = warp_sum(sAbsR);
+      Egas_new = Egas_t - c_over_chat * sR;
+      // ---- a7: closure + flux update with the lagged velocity (Eq. 51); a8: gas momentum (Eq. 52) ----
+      double dF0 = 0.0, dF1 = 0.0, dF2 = 0.0;
+      bool rel_ok = true;
+#pragma unroll
+      for (int k = 0; k < GPL; ++k) {
+        double p0, p1, p2;
+        closure_vP(P.closure, Enew[k], Fk0[k], Fk1[k], Fk2[k], v0, v1, v2, c, p0, p1, p2);
+        const double w = (1.0 + alpha[k]) * chiE[k];
+        const double dn = fma(cdt, chiF[k], 1.0);
+        Fn0[k] = fma(cdt, fma(v0, AG[k], w * p0), Ft0[k]) / dn;
+        Fn1[k] = fma(cdt, fma(v1, AG[k], w * p1), Ft1[k]) / dn;
+        Fn2[k] = fma(cdt, fma(v2, AG[k], w * p2), Ft2[k]) / dn;
+        if (vg[k]) {
+          dF0 += Fn0[k] - Ft0[k]; dF1 += Fn1[k] - Ft1[k]; dF2 += Fn2[k] - Ft2[k];
+          if (P.outer_stop == 1 &&
+              !(norm3(Fn0[k] - Fk0[k], Fn1[k] - Fk1[k], Fn2[k] - Fk2[k]) <= P.outer_rel_tol * norm3(Fn0[k], Fn1[k], Fn2[k])))
+            rel_ok = false;
+        }
+      }
+      dF0 = warp_sum(dF0); dF1 = warp_sum(dF1); dF2 = warp_sum(dF2);
+      momn0 = momt0 - dF0 * icc; momn1 = momt1 - dF1 * icc; momn2 = momt2 - dF2 * icc;
+      trips++;
+      // ---- a9: outer test (reading S10) ------------------------------------------------
+      const double vn0 = momn0 * inv_rho, vn1 = momn1 * inv_rho, vn2 = momn2 * inv_rho;
+      double dW = 0.0;
+#pragma unroll
+      for (int k = 0; k < GPL; ++k) {
+        const double vFn = fma(vn0, Fn0[k], fma(vn1, Fn1[k], vn2 * Fn2[k]));
+        const double Wn = (1.0 + alpha[k]) * chiF[k] * vFn / c;
+        if (vg[k]) dW += fabs(Wn - W[k]);
+      }
+      dW = warp_sum(dW);
+      rel_ok = __all_sync(FULL, rel_ok);
+      if (P.outer_stop == 1 &&
+          !(norm3(momn0 - momk0, momn1 - momk1, momn2 - momk2) <= P.outer_rel_tol * norm3(momn0, momn1, momn2)))
+        rel_ok = false;
+      const double delta = dW * (chat / c) * dt;
+      if (delta <= P.outer_tol * fmax(sAbsR, Etot) && rel_ok) break;
+      if (kk == P.outer_maxit - 1) {
+        if (lane == 0) atomicAdd(&stats[kStatOuterUnconv], 1ull);
+        break;
+      }
+      momk0 = momn0; momk1 = momn1; momk2 = momn2;
+#pragma unroll
+      for (int k = 0; k < GPL; ++k) { Fk0[k] = Fn0[k]; Fk1[k] = Fn1[k]; Fk2[k] = Fn2[k]; }
+    }
+
+    // ---- a10: store in place ------------------------------------------------------------------------
+    if (trips > 0) {
+      if (lane == 0) {
+        S.mom[0][cell] = momn0; S.mom[1][cell] = momn1; S.mom[2][cell] = momn2;
+        S.Egas[cell] = Egas_new;     // total gas energy; E_int = Egas - |mom|^2/(2 rho)
+      }
+#pragma unroll
+      for (int k = 0; k < GPL; ++k)
+        if (vg[k]) {
+          const long long o = (long long)gi[k] * stride + cell;
+          S.Erad[o] = Enew[k];
+          S.Frad[0][o] = Fn0[k]; S.Frad[1][o] = Fn1[k]; S.Frad[2][o] = Fn2[k];
+        }
+    }
+    if (lane == 0) {
+      atomicAdd(&s_cnt[GS_EVALS], (unsigned)evals);
+      atomicAdd(&s_cnt[GS_TRIPS], (unsigned)trips);
+      atomicAdd(&s_hist[evals < MGRHD_HIST ? evals : MGRHD_HIST - 1], 1u);
+      atomicAdd(&s_hist[MGRHD_HIST + (trips < MGRHD_HIST ? trips : MGRHD_HIST - 1)], 1u);
+    }
+  }
+
+  __syncthreads();
+  if (threadIdx.x < GS_COUNT && s_cnt[threadIdx.x]) {
+    const int t = threadIdx.x;
+    const int slot = t == GS_EVALS ? kStatNewtonEvals : (t == GS_TRIPS ? kStatOuterTrips : (t == GS_GUARD ? kStatChiFGuard : kStatDenNonPos));
+    atomicAdd(&stats[slot], (unsigned long long)s_cnt[t]);
+  }
+  for (int t = threadIdx.x; t < 2 * MGRHD_HIST; t += blockDim.x)
+    if (s_hist[t]) {
+      atomicAdd(&stats[kStatNewtonHist + t], (unsigned long long)s_hist[t]);
+      if (t < MGRHD_HIST) atomicAdd(&stats[kStatCells], (unsigned long long)s_hist[t]);
+    }
+}
+
+}  // namespace mgrhd

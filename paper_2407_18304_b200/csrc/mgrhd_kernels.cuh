@@ -150,7 +150,9 @@ __device__ __forceinline__ double cell_sum(double v) {
 //         stores that cell's E_g here, so none of these costs a loop of its own;
 //   B, C  cells whose Newton iteration converged do the flux/momentum update and the outer test
 //         (a6-a9); F_g is updated in place in the state, so a finished cell needs no flux store.
-template <int L, int NQL, int THREADS, bool COUNT>
+// KT: opacity_kind 1 -- chi_{g-} = rho s kappa_lo[g] (T/T_ref)^p_T at every trial temperature
+//    (PAPER.md:499): all opacities of a cell carry the one factor, so it multiplies the per-cell `chis`.
+template <int L, int NQL, int THREADS, bool KT, bool COUNT>
 __global__ void __launch_bounds__(THREADS, 1)
 source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ StatePtrs S,
                      unsigned long long* __restrict__ stats, double* __restrict__ scratch0) {
@@ -232,6 +234,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
   int phase = PH_LOAD;
   long long cell = 0, fin_cell = -1;   // fin_cell: finished cell whose E_g store is still due
   double rho = 1.0, inv_rho = 1.0, chis = 1.0, inv_chis = 1.0, inv_Cv = 1.0, Egas_t = 0.0, Etot = 1.0;
+  double chis0 = 1.0, inv_chis0 = 1.0;   // KT: chis at T_ref; chis, inv_chis then hold the values at the last trial T
   double momt0 = 0, momt1 = 0, momt2 = 0, momk0 = 0, momk1 = 0, momk2 = 0;
   double Egs = 0.0, Ekin = 0.0, lam = 0.0, ldx = 0.0;
   bool first = false, pend = false;
@@ -286,6 +289,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
         Egas_t = S.Egas[cell];
         chis = rho * ks;                      // chi_{g-} = chis * k_lo[g]
         inv_chis = 1.0 / chis;
+        if (KT) { chis0 = chis; inv_chis0 = inv_chis; }
         inv_rho = 1.0 / rho;
         inv_Cv = 1.0 / (rho * P.cv_over_rho);
         momk0 = momt0; momk1 = momt1; momk2 = momt2;
@@ -318,6 +322,10 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
       const double T2 = T * T;
       const double aT4 = P.a_rad * T2 * T2;
       const double beta = P.h_over_k * invT;
+      if (KT) {                                         // opacities at this trial temperature
+        const double f = pow(T * P.inv_T_ref, P.p_T);
+        if (ev) { chis = chis0 * f; inv_chis = inv_chis0 / f; }
+      }
       const double itau_c = inv_chis * inv_cdt;         // 1/(c_hat dt chi_E,g) = itau_c * inv_k_mean[g]
       const double jscale = aT4 * invT * inv_Cv;     // J_g0 = (4 Bt - Db) / (T C_v), Eq. 46, per unit (4 dY - dXi)
       const double wscale = inv_chis * inv_c * inv_c; // W_g/(c chi_E) = (1+alpha)/k_mean chi_F v.F wscale
@@ -340,6 +348,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
       const int src = sub == 0 ? lane + (L - 1) : lane - 1;   // lane that owns the lower edge
       const bool last = sub == L - 1;
       const bool evf = ev && first, evp = ev && pend;
+      const bool anyf = __any_sync(FULL, evf);
       // register prefetch of the next step's global operands (group g = i*L + sub).
       // Byte offsets of (group, cell) advance by a warp-uniform stride per step, so each stream
       // costs one 64-bit add and one load.
@@ -347,6 +356,9 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
       const char* const pF0 = reinterpret_cast<const char*>(S.Frad[0]);
       const char* const pF1 = reinterpret_cast<const char*>(S.Frad[1]);
       const char* const pF2 = reinterpret_cast<const char*>(S.Frad[2]);
+      // S_g enters Eq. 41, Eq. 50 and the commit only through E_g^(t) + S_g: the first
+      // evaluation of a cell adds it to the state's E_g in place (warp-uniform test: no cost without sources)
+      const bool srcs = S.Srad != nullptr && anyf;
       const long long dstep = (long long)L * stride * 8;
       long long oc = ((long long)sub * stride + cell) * 8;        // (g, cell) of the step being loaded
       long long of = ((long long)sub * stride + fin_cell) * 8;    // (g, fin_cell)
@@ -369,7 +381,15 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
         const int e = g + 1;                         // its upper edge
         const bool vg = g < Nq;
         const bool evg = ev && vg;
-        const double Et = nEt, F0 = nF0, F1 = nF1, F2 = nF2, Eo = nEo;
+        double Et = nEt;
+        const double F0 = nF0, F1 = nF1, F2 = nF2, Eo = nEo;
+        if (srcs) {
+          if (evf && vg) {
+            MGRHD_CHK(oc >= 0 && oc < lim_state);
+            Et += ldd(reinterpret_cast<const char*>(S.Srad), oc);
+            *reinterpret_cast<double*>(const_cast<char*>(pE) + oc) = Et;
+          }
+        }
         of_cur = of;
         oc += dstep;
         of += dstep;
@@ -451,8 +471,8 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
       // the arrowhead reductions of Eq. 48 and the sums of Eq. 49-50 across the lanes of the cell
       sumR = cell_sum<L>(sumR); sumAbsFR = cell_sum<L>(sumAbsFR);
       SFRq = cell_sum<L>(SFRq); SJq = cell_sum<L>(SJq);
-      if (__any_sync(FULL, ev && first)) sumEt = cell_sum<L>(sumEt);
-      if (COUNT && ev) flops += (unsigned)eflops + (sub == 0 ? kFlopCellEval + kFlopGroupEval * Nq : 0);
+      if (anyf) sumEt = cell_sum<L>(sumEt);
+      if (COUNT && ev) flops += (unsigned)eflops + (sub == 0 ? kFlopCellEval + (KT ? kFlopPowT : 0) + kFlopGroupEval * Nq : 0);
       // 1/(1 - sum J0g Jg0/Jgg) of the gas-row elimination (>= 1 for any physical state), formed warp-wide
       const double inv_jd = warp_rcp(fma(c_over_chat, SJq, 1.0));
       if (ev) {

@@ -44,6 +44,7 @@ constexpr int kFlopStepCell = 10;     // dx0, T > 0 check, E_gas update
 constexpr int kFlopStepGroup = 4;     // R_g += lam da_g + (lam dx0) db_g
 constexpr int kFlopOuterCell = 50;    // v, Eq. 52, commit, E_kin, outer tests, sums over the cell's lanes
 constexpr int kFlopOuterGroup = 102;  // closure (46), Eq. 51 (23), relative-change test (14), sums (9), next v.F_g and dW (10)
+constexpr int kFlopPowT = 64;         // opacity_kind 1: (T/T_ref)^p_T = exp(p ln(.)) (log 30, exp 30), chis, 1/chis
 constexpr int kFlopCell = 16;         // load-time derivations
 constexpr int kFlopCellGroup = 7;     // sum E_g, first v.F_g, E_g commit
 
@@ -65,6 +66,8 @@ struct Params {
   double inv_k_mean[kMaxG]; // 1 / k_mean[g]
   double k_num[kMaxG];      // k_mean[g] * (4 + alpha_g)/3 : numerator factor of Eq. 27 with chi_B = chi_E
   double onepa[kMaxG];      // 1 + alpha_g (Eq. 21, 22)
+  // ---- opacity_kind 1: chi scales with (T / T_ref)^p_T at every trial temperature ----
+  double inv_T_ref, p_T;
   // ---- per call ------------------------------------------------------------------
   double dt, c, c_hat;
   long long ncells;   // cells in this launch
@@ -78,6 +81,20 @@ struct StatePtrs {
   double* Erad;
   double* Frad[3];
   const double* kappa_scale;  // may be null
+  const double* Srad;         // S_g [Nq][n], may be null
+};
+
+// Extra parameters of the general kernel (mgrhd_general.cuh): group geometry for Eq. 30 and Eq. A1-A2,
+// the spectrum / opacity switches and the edge-opacity table of opacity_kind 2 (device memory).
+struct GenParams {
+  int spectrum;             // 0 fixed slope alpha_Q = -1, 1 free slope (Appendix A)
+  int opacity_kind;         // 0, 1, 2 as in mgrhd_opacity_model
+  int NT;
+  double lnT0, inv_dlnT;
+  const double* lnk_edge;   // device, [Nq+1][NT]
+  double lnr[kMaxG];        // ln(nu_g+ / nu_g-); 0 for a group with an edge at 0 or +inf
+  double width[kMaxG];      // nu_g+ - nu_g-  (Qbar_g = Q_g / width, Eq. A1)
+  double inv_lnnb[kMaxG];   // 1 / ln(nubar_{g+1} / nubar_g), nubar = sqrt(nu_g+ nu_g-); 0 where Eq. A1 is undefined
 };
 
 // Tables of the Planck edge functions (mgrhd_planck.cuh), filled by the host once per device

@@ -40,7 +40,8 @@ def test_every_declared_symbol_is_exported(binding):
 def test_struct_layouts_match_header(binding):
     """ctypes mirrors: field counts/sizes implied by the header."""
     assert ctypes.sizeof(binding.Units) == 5 * 8
-    assert ctypes.sizeof(binding.State) == 10 * 8
+    assert ctypes.sizeof(binding.State) == 11 * 8            # ... + Srad
+    assert ctypes.sizeof(binding.OpacityModel) == 120        # 2 pointers, controls, then kind / T_ref / p_T / NT / lnT0 / dlnT / table
     assert ctypes.sizeof(binding.Stats) == (9 + 2 * 64) * 8
     src = open(HEADER).read()
     assert "#define MGRHD_MAX_GROUPS 64" in src and "#define MGRHD_HIST 64" in src
@@ -73,7 +74,22 @@ def test_init_argument_errors(binding):
     with pytest.raises(binding.MgrhdError, match="MGRHD_ERR_ARG"):
         _init(binding, e, k, a, closure=2)
     with pytest.raises(binding.MgrhdError, match="MGRHD_ERR_ARG"):
-        _init(binding, e, k, a, spectrum=1)           # free-slope fit is not built
+        _init(binding, e, k, a, spectrum=2)
+    with pytest.raises(binding.MgrhdError, match="MGRHD_ERR_ARG"):
+        _init(binding, e, k, a, opacity_kind=3)
+    with pytest.raises(binding.MgrhdError, match="MGRHD_ERR_RANGE"):
+        _init(binding, e, k, a, opacity_kind=1, T_ref=0.0, p_T=1.5)
+    with pytest.raises(binding.MgrhdError, match="MGRHD_ERR_ARG"):
+        _init(binding, e, None, None, opacity_kind=2)                                   # no table
+    tab = np.zeros((3, 4))
+    with pytest.raises(binding.MgrhdError, match="MGRHD_ERR_ALPHA"):
+        _init(binding, np.array([0.0, 2.0, 4.0]), None, None, opacity_kind=2, lnk_edge=tab)   # Eq. 20 needs finite edges > 0
+    with pytest.raises(binding.MgrhdError, match="MGRHD_ERR_RANGE"):
+        _init(binding, e, None, None, opacity_kind=2, lnk_edge=tab, dlnT=0.0)
+    bad = tab.copy()
+    bad[1, 2] = np.nan
+    with pytest.raises(binding.MgrhdError, match="MGRHD_ERR_RANGE"):
+        _init(binding, e, None, None, opacity_kind=2, lnk_edge=bad)
     with pytest.raises(binding.MgrhdError, match="MGRHD_ERR_ARG"):
         _init(binding, np.arange(67.0) + 1, np.ones(66), np.zeros(66))   # Nq > MGRHD_MAX_GROUPS
 
