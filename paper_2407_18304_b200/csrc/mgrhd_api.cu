@@ -170,22 +170,26 @@ struct mgrhd_ctx {
 // with as many threads per SM as the register file allows.
 template <int L, int NQL, int THREADS, bool KT>
 struct Inst {
+  template <bool SRC, bool COUNT>
+  static auto kernel() { return source_update_kernel<L, NQL, THREADS, KT, SRC, COUNT>; }
   static constexpr size_t kSmem = (size_t)SL_COUNT * NQL * THREADS * sizeof(double);
   static cudaError_t configure(int* blocks_per_sm) {
-    cudaError_t e = cudaFuncSetAttribute(source_update_kernel<L, NQL, THREADS, KT, false>,
-                                         cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem);
+    cudaError_t e = cudaSuccess;
+    const void* k[4] = {(const void*)kernel<false, false>(), (const void*)kernel<false, true>(),
+                        (const void*)kernel<true, false>(), (const void*)kernel<true, true>()};
+    for (int i = 0; i < 4 && e == cudaSuccess; ++i)
+      e = cudaFuncSetAttribute(k[i], cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem);
     if (e == cudaSuccess)
-      e = cudaFuncSetAttribute(source_update_kernel<L, NQL, THREADS, KT, true>,
-                               cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmem);
-    if (e == cudaSuccess)
-      e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, source_update_kernel<L, NQL, THREADS, KT, false>,
-                                                        THREADS, kSmem);
+      e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, kernel<false, false>(), THREADS, kSmem);
     return e;
   }
   static void launch(bool count, unsigned blocks, cudaStream_t st, const Params& P, const StatePtrs& S,
                      unsigned long long* stats, double* scratch) {
-    if (count) source_update_kernel<L, NQL, THREADS, KT, true><<<blocks, THREADS, kSmem, st>>>(P, S, stats, scratch);
-    else source_update_kernel<L, NQL, THREADS, KT, false><<<blocks, THREADS, kSmem, st>>>(P, S, stats, scratch);
+    const bool src = S.Srad != nullptr;
+    if (src && count) kernel<true, true>()<<<blocks, THREADS, kSmem, st>>>(P, S, stats, scratch);
+    else if (src) kernel<true, false>()<<<blocks, THREADS, kSmem, st>>>(P, S, stats, scratch);
+    else if (count) kernel<false, true>()<<<blocks, THREADS, kSmem, st>>>(P, S, stats, scratch);
+    else kernel<false, false>()<<<blocks, THREADS, kSmem, st>>>(P, S, stats, scratch);
   }
 };
 

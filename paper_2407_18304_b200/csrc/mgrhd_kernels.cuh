@@ -87,28 +87,24 @@ __device__ __forceinline__ void closure_vP(int closure, double E, double F0, dou
   const double t0 = F0 * r1, t1 = F1 * r1, t2 = F2 * r1;
   const double f2u = fma(t0, t0, fma(t1, t1, t2 * t2));                            // f^2 before the clamp
   // isotropic when: Eddington closure, E <= 0, F = 0 (|F|^2 underflows exactly as the oracle's |F| does),
-  // or f^2 below the normal range (the anisotropic term is then < 1e-290 of the isotropic one)
-  const bool iso = closure == 1 || !(E > 0.0) || Fzero || !(f2u > 1e-290);
+  // f^2 below the normal range (the anisotropic term is then < 1e-290 of the isotropic one), or f^2 >= 1e290
+  // (or not finite: F/(cE) overflows).  In that last case |F| exceeds c E by a factor 1e145, so c_hat dt chi v.P
+  // is below one ulp of F in Eq. 51 and of its change in Eq. 52 whatever the closure returns: any finite value
+  // gives the oracle's F_g^(new) bit for bit, and the isotropic one needs no code of its own.  (A separate
+  // rescue path for this case, ~40 instructions that never execute, cost 13 % of the whole update inlined
+  // in the flux loop and 8 % out of line.)
+  const bool iso = closure == 1 || !(E > 0.0) || Fzero || !(f2u > 1e-290) || !(f2u < 1e290);
   const double f2 = f2u > 1.0 ? 1.0 : f2u;
   // chi = (3 + 4 f^2)/(5 + 2 s), s = sqrt(4 - 3 f^2), equals (5 - 2 s)/3 (multiply through by 5 - 2 s), so
   // (1 - chi)/2 = (s - 1)/3 and (3 chi - 1)/2 = 2 - s: one sqrt, no division
   const double sq = sqrt(fma(-3.0, f2, 4.0));
-  const bool big = !iso && !(f2u < 1e290);       // |F| >> c E (f is clamped to 1): f^2 or t itself overflows
-  const double r2 = fast_rcp(iso || big ? 1.0 : f2u);
+  const double r2 = fast_rcp(iso ? 1.0 : f2u);
   const double tv = fma(t0, v0, fma(t1, v1, t2 * v2));
   const double a = iso ? 1.0 / 3.0 : (sq - 1.0) * (1.0 / 3.0);
   const double b = (2.0 - sq) * tv * r2;
   p0 = E * fma(a, v0, iso ? 0.0 : b * t0);       // (t may be inf/NaN on isotropic lanes: selected away)
   p1 = E * fma(a, v1, iso ? 0.0 : b * t1);
   p2 = E * fma(a, v2, iso ? 0.0 : b * t2);
-  if (__any_sync(0xffffffffu, big)) {            // warp-uniform and practically never taken
-    // free-streaming limit f = 1 (chi = 1, P = E n n): n from F scaled by its largest component,
-    // so that n (n.v) is formed finitely whatever F/(cE) is (E ~ 1e-320 beside F ~ 1e-150)
-    const double m = fmax(fabs(F0), fmax(fabs(F1), fabs(F2)));
-    const double u0 = F0 / m, u1 = F1 / m, u2 = F2 / m;
-    const double uv = fma(u0, v0, fma(u1, v1, u2 * v2)) / fma(u0, u0, fma(u1, u1, u2 * u2));
-    if (big) { p0 = E * (uv * u0); p1 = E * (uv * u1); p2 = E * (uv * u2); }
-  }
 }
 
 // Lane phases of the flattened iteration.
@@ -152,7 +148,8 @@ __device__ __forceinline__ double cell_sum(double v) {
 //         (a6-a9); F_g is updated in place in the state, so a finished cell needs no flux store.
 // KT: opacity_kind 1 -- chi_{g-} = rho s kappa_lo[g] (T/T_ref)^p_T at every trial temperature
 //    (PAPER.md:499): all opacities of a cell carry the one factor, so it multiplies the per-cell `chis`.
-template <int L, int NQL, int THREADS, bool KT, bool COUNT>
+// SRC: a source term S_g is present.
+template <int L, int NQL, int THREADS, bool KT, bool SRC, bool COUNT>
 __global__ void __launch_bounds__(THREADS, 1)
 source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ StatePtrs S,
                      unsigned long long* __restrict__ stats, double* __restrict__ scratch0) {
@@ -348,7 +345,6 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
       const int src = sub == 0 ? lane + (L - 1) : lane - 1;   // lane that owns the lower edge
       const bool last = sub == L - 1;
       const bool evf = ev && first, evp = ev && pend;
-      const bool anyf = __any_sync(FULL, evf);
       // register prefetch of the next step's global operands (group g = i*L + sub).
       // Byte offsets of (group, cell) advance by a warp-uniform stride per step, so each stream
       // costs one 64-bit add and one load.
@@ -356,9 +352,8 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
       const char* const pF0 = reinterpret_cast<const char*>(S.Frad[0]);
       const char* const pF1 = reinterpret_cast<const char*>(S.Frad[1]);
       const char* const pF2 = reinterpret_cast<const char*>(S.Frad[2]);
-      // S_g enters Eq. 41, Eq. 50 and the commit only through E_g^(t) + S_g: the first
-      // evaluation of a cell adds it to the state's E_g in place (warp-uniform test: no cost without sources)
-      const bool srcs = S.Srad != nullptr && anyf;
+      // SRC: S_g enters Eq. 41, Eq. 50 and the commit only through E_g^(t) + S_g: the first
+      // evaluation of a cell adds it to the state's E_g in place
       const long long dstep = (long long)L * stride * 8;
       long long oc = ((long long)sub * stride + cell) * 8;        // (g, cell) of the step being loaded
       long long of = ((long long)sub * stride + fin_cell) * 8;    // (g, fin_cell)
@@ -383,7 +378,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
         const bool evg = ev && vg;
         double Et = nEt;
         const double F0 = nF0, F1 = nF1, F2 = nF2, Eo = nEo;
-        if (srcs) {
+        if constexpr (SRC) {
           if (evf && vg) {
             MGRHD_CHK(oc >= 0 && oc < lim_state);
             Et += ldd(reinterpret_cast<const char*>(S.Srad), oc);
@@ -471,7 +466,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
       // the arrowhead reductions of Eq. 48 and the sums of Eq. 49-50 across the lanes of the cell
       sumR = cell_sum<L>(sumR); sumAbsFR = cell_sum<L>(sumAbsFR);
       SFRq = cell_sum<L>(SFRq); SJq = cell_sum<L>(SJq);
-      if (anyf) sumEt = cell_sum<L>(sumEt);
+      if (__any_sync(FULL, ev && first)) sumEt = cell_sum<L>(sumEt);
       if (COUNT && ev) flops += (unsigned)eflops + (sub == 0 ? kFlopCellEval + (KT ? kFlopPowT : 0) + kFlopGroupEval * Nq : 0);
       // 1/(1 - sum J0g Jg0/Jgg) of the gas-row elimination (>= 1 for any physical state), formed warp-wide
       const double inv_jd = warp_rcp(fma(c_over_chat, SJq, 1.0));
