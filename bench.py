@@ -39,6 +39,9 @@ def parse_args():
     ap.add_argument("--sustained", type=int, default=0, metavar="CALLS",
                     help="BASELINE.json config 5 as stated: CALLS successive updates of the same buffers, dt varied "
                          "per call, device-timed per call, conservation residuals checked after every call")
+    ap.add_argument("--variant", default="default", choices=["default", "source", "ktemp", "free_slope", "edge_table"],
+                    help="model option on top of the workload (SURVEY 8(f) rows): S_g present; kappa (T/T_ref)^1.5; "
+                         "free-slope spectrum fit; edge opacities tabulated in T with alpha from Eq. 20")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -101,10 +104,11 @@ class ClockSampler:
 # CPU oracle legs (the only places bench.py touches oracle/)
 # --------------------------------------------------------------------------------------
 def oracle_model(oracle, wl):
+    extra = {k: getattr(wl, k) for k in ("spectrum", "opacity_kind", "T_ref", "p_T", "lnT0", "dlnT", "lnk_edge") if hasattr(wl, k)}
     return oracle.OracleModel(wl.edges, wl.kappa_lo, wl.alpha, a_rad=wl.a_rad, k_B=wl.k_B, h_planck=wl.h_planck,
                               mean_mass=wl.mean_mass, gamma=wl.gamma, closure=wl.closure, newton_tol=wl.newton_tol,
                               newton_maxit=wl.newton_maxit, outer_maxit=wl.outer_maxit, outer_tol=wl.outer_tol,
-                              outer_stop=wl.outer_stop, outer_rel_tol=wl.outer_rel_tol)
+                              outer_stop=wl.outer_stop, outer_rel_tol=wl.outer_rel_tol, **extra)
 
 
 def default_cpu_sample(wl) -> int:
@@ -130,9 +134,13 @@ def run_reference(args) -> None:
         return
     from paper_2407_18304_b200 import workloads as W
 
-    wl = W.workload(args.workload, ncells=args.cells)
+    wl = apply_variant(W.workload(args.workload, ncells=args.cells), args.variant)
     sample = min(wl.ncells, args.cpu_sample_cells or max(1024, default_cpu_sample(wl) // 4))
     st0 = W.to_numpy(wl.make_state(ncells=sample))
+    if args.variant == "source":
+        import numpy as np
+
+        st0["Srad"] = st0["Erad"] * np.random.default_rng(1234).uniform(0.0, 2.0, st0["Erad"].shape)
     times = []
     for step in range(args.warmup + args.steps):
         st = {k: (None if v is None else v.copy()) for k, v in st0.items()}
@@ -152,6 +160,54 @@ def run_reference(args) -> None:
         "gpu_launches": 0,
     }
     print(json.dumps(line))
+
+
+def apply_variant(wl, variant: str):
+    """Model options of SURVEY 8(f) on the shapes of the BASELINE workloads (same state recipe)."""
+    import math
+
+    import numpy as np
+
+    if variant == "ktemp":                     # PAPER.md:499, Marshak (c): chi_g (T/T_0)^{3/2}
+        wl.opacity_kind, wl.T_ref, wl.p_T = 1, 1.0, 1.5
+    elif variant == "free_slope":              # Appendix A
+        wl.spectrum = 1
+    elif variant == "edge_table":              # Eq. 20 on a continuous opacity kappa ~ nu^-1.5 T^-0.5 (free-free-like, cf. Eq. 62)
+        lnT = np.linspace(math.log(1e-2), math.log(1e2), 33)
+        k_edge = wl.edges ** -1.5
+        wl.opacity_kind = 2
+        wl.lnk_edge = np.log(k_edge)[:, None] - 0.5 * lnT[None, :]
+        wl.lnT0, wl.dlnT = float(lnT[0]), float(lnT[1] - lnT[0])
+    if variant != "default":
+        wl.name = f"{wl.name}+{variant}"
+    return wl
+
+
+def kernel_source_sha() -> str:
+    """sha256 over the CUDA sources: ties an ncu traffic figure under profiles/ to the kernel it was taken from."""
+    import hashlib
+
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_2407_18304_b200", "csrc")
+    for name in sorted(os.listdir(d)):
+        h.update(open(os.path.join(d, name), "rb").read())
+    return h.hexdigest()[:16]
+
+
+def ncu_traffic(workload_name: str, cells: int):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the update kernel from the `ncu --set full`
+    capture recorded in profiles/traffic.csv (workload, cells, read bytes, write bytes, kernel source sha, file),
+    scaled linearly to `cells` (persistent grid-stride kernel).  None when there is no capture of this
+    workload taken from the kernel sources as they are now."""
+    path = os.path.join(ROOT, "profiles", "traffic.csv")
+    if not os.path.exists(path):
+        return None, None
+    sha = kernel_source_sha()
+    for line in open(path):
+        f = [t.strip() for t in line.split(",")]
+        if len(f) >= 6 and f[0] == workload_name and f[4] == sha:
+            return (float(f[2]) + float(f[3])) * cells / float(f[1]), f[5]
+    return None, None
 
 
 # --------------------------------------------------------------------------------------
@@ -190,6 +246,9 @@ def run_ours(args) -> None:
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}: launch with torch.distributed.run "
+                         f"--nproc-per-node {args.gpus} (a plain `python bench.py --gpus N` spawns it itself)")
     assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
     torch.cuda.set_device(local)
     if world > 1:
@@ -200,12 +259,20 @@ def run_ours(args) -> None:
         dist.barrier()
     binding.load_library()
 
-    wl = W.workload(args.workload, ncells=args.cells)
+    wl = apply_variant(W.workload(args.workload, ncells=args.cells), args.variant)
     n, Nq = wl.ncells, wl.Nq
     dt = wl.dt_of_call(0)
     # weak scaling: every rank updates its own n cells (disjoint seeded cell ranges); no collective on the data path
     pristine = wl.make_state(device="cuda", cell_start=rank * n, ncells=n)
+    if args.variant == "source":               # S_g = E_g^(t) x U[0, 2) (seeded)
+        g = torch.Generator(device="cuda").manual_seed(1234 + rank)
+        pristine["Srad"] = pristine["Erad"] * (2.0 * torch.rand(pristine["Erad"].shape, generator=g, device="cuda", dtype=torch.float64))
     work = alloc_like(pristine)
+    # L2: a state well above the 126 MB L2 evicts itself (and is restored from the pristine copy before every
+    # step, another full sweep); smaller states get an explicit flush -- a 512 MB write -- before every timed step
+    flush = None
+    if state_nbytes(pristine) < (512 << 20):
+        flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")
     ctx = binding.Context.from_workload(wl)
     stream = torch.cuda.current_stream()
 
@@ -227,6 +294,8 @@ def run_ours(args) -> None:
     stats = ctx.get_stats()
     ctx.set_flop_counting(False)
     ctx.conserved_totals(work, wl.c, wl.c_hat, E1, P1)
+    if pristine.get("Srad") is not None:       # E_gas + (c/c_hat) sum (E_g - S_g) is what is conserved
+        E0 += (wl.c / wl.c_hat) * pristine["Srad"].sum(0)
     Es = pristine["Egas"].abs() + (wl.c / wl.c_hat) * pristine["Erad"].abs().sum(0)
     resE = float(((E1 - E0).abs() / Es).max())
     Ps = pristine["mom"].pow(2).sum(0).sqrt() + pristine["Frad"].pow(2).sum(0).sqrt().sum(0) / (wl.c * wl.c_hat)
@@ -248,6 +317,8 @@ def run_ours(args) -> None:
     evs = []
     for _ in range(args.steps):
         copy_state(work, pristine)           # untimed restore (also evicts the previous step from L2)
+        if flush is not None:
+            flush.fill_(1)                   # L2 flush for states that would otherwise stay resident
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record(stream)
         ctx.source_update(work, dt, wl.c, wl.c_hat)
@@ -269,17 +340,22 @@ def run_ours(args) -> None:
     peak_tflops = 2.0 * dfma / 1e12
     avg_launch_s = (sum(step_ms) / len(step_ms)) * 1e-3
     achieved_tflops = flops_per_launch / avg_launch_s / 1e12
-    alg_bytes = 8.0 * n * ((5 + 4 * Nq) + (4 + 4 * Nq) + (0 if pristine["kappa_scale"] is None else 1))
+    alg_bytes = 8.0 * n * ((5 + 4 * Nq) + (4 + 4 * Nq) + (0 if pristine["kappa_scale"] is None else 1)
+                           + (Nq if pristine.get("Srad") is not None else 0))
+    traffic, traffic_src = ncu_traffic(workload_label(wl), n)
     peaks = {}
     try:
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
     except Exception:
         pass
     hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
+    counted = flops_per_launch > 0            # the general kernel (free slope, edge table) is not instrumented
     roofline = {
-        "bound": "alu", "achieved": achieved_tflops, "peak": peak_tflops, "unit": "TFLOP/s",
-        "frac": achieved_tflops / peak_tflops,
-        "traffic": NCU_TRAFFIC_BYTES.get(wl.index) if n == W.workload(wl.index).ncells else None,
+        "bound": "alu", "achieved": achieved_tflops if counted else None, "peak": peak_tflops, "unit": "TFLOP/s",
+        "frac": achieved_tflops / peak_tflops if counted else None,
+        "note": None if counted else "general kernel (one warp per cell): algorithmic flops not instrumented; see the HBM figures",
+        "traffic": traffic,
+        "traffic_source": traffic_src and f"profiles/{traffic_src} (ncu --set full, scaled linearly in cells; kernel sources sha {kernel_source_sha()})",
         "peak_source": "FP64 FMA rate measured in this run by mgrhd_measure_dfma_peak (x2 flop/FMA)",
         "algorithmic_flops_per_launch": flops_per_launch,
         "algorithmic_flops_per_cell_group": flops_per_launch / (n * Nq),
@@ -294,7 +370,10 @@ def run_ours(args) -> None:
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": workload_label(wl), "cells_per_gpu": n, "Nq": Nq, "dt": dt, "c": wl.c,
                    "c_hat": wl.c_hat, "newton_tol": wl.newton_tol, "outer_stop": wl.outer_stop,
-                   "l2": "state (%.2f GB) larger than L2; restored from a pristine copy before every step"
+                   "variant": args.variant,
+                   "l2": ("state (%.3f GB) larger than L2; restored from a pristine copy before every step"
+                          if flush is None else
+                          "state (%.3f GB) fits in or near L2: flushed by a 512 MB write before every timed step")
                          % (state_nbytes(pristine) / 1e9)},
         "clocks": clocks, "gpu_launches": gpu_launches, "roofline": roofline,
         "step_ms": step_ms,
@@ -323,13 +402,6 @@ def run_ours(args) -> None:
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
-
-
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the update kernel, from the
-# `ncu --set full` capture summarised in profiles/r1_final_ncu_full.md: 2.678 + 6.115 GB at
-# 2 097 152 cells of config 4, scaled x8 to its 16 777 216 cells (persistent grid-stride kernel,
-# traffic linear in cells).  None for workloads without a capture.
-NCU_TRAFFIC_BYTES: dict = {4: 8.0 * (2.895354e9 + 5.651977e9)}
 
 
 def run_e2e(args, wl, ctx, pristine, dt, world, dist):
@@ -374,26 +446,52 @@ def run_e2e(args, wl, ctx, pristine, dt, world, dist):
             "host_memory": "pinned"}
 
 
+def cpu_sample_plan(args, wl):
+    """(cells per slab, slabs): one slab per host core, each about half the single-core sample."""
+    cores = max(1, len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1))
+    M = min(wl.ncells, max(256, (args.cpu_sample_cells or default_cpu_sample(wl)) // 2))
+    return M, max(1, min(cores, wl.ncells // M)), cores
+
+
 def run_cpu_baseline(args, wl, pristine, work, dt):
-    """Oracle on the first M cells (one host core), and parity of the GPU result on the same cells."""
+    """The oracle as it stands on a bounded sample of the same state: first on ONE host core (M cells), then on
+    ALL host cores (one thread per core, each its own slab of M cells, no shared state), and parity of the GPU
+    result on every cell the oracle computed."""
+    from concurrent.futures import ThreadPoolExecutor
+
     import numpy as np
-    import torch
 
     sys.path.insert(0, os.path.join(ROOT, "tests"))
-    from parity_util import compare
+    from parity_util import afloor_quasi_newton, compare
 
     from paper_2407_18304_b200 import workloads as W
 
-    M = min(wl.ncells, args.cpu_sample_cells or default_cpu_sample(wl))
-    st0 = W.to_numpy({k: (None if v is None else v[..., :M]) for k, v in pristine.items()})
-    ref = {k: (None if v is None else v.copy()) for k, v in st0.items()}
-    secs, ost = time_oracle(wl, ref, dt)
-    got = W.to_numpy({k: (None if v is None else v[..., :M]) for k, v in work.items()})   # last timed step's result
-    res = compare(ref, got, st0, wl.c, wl.c_hat)
-    cpu = {"value": M * wl.Nq / secs, "unit": UNIT, "cores": 1, "kind": "oracle",
-           "sample": f"first {M} cells of {workload_label(wl)}, one update, single thread, dense LU", "seconds": secs,
-           "host_cores_available": os.cpu_count()}
-    parity = {"cells": M, "tolerance": "|d| <= 1e-10|ref| + 1e-14 S_cell", "ok": all(v[0] == 0 for v in res.values()),
+    M, slabs, cores = cpu_sample_plan(args, wl)
+    # pristine / work: device or host state dicts whose first M*slabs cells are U^(t) and the GPU's U^(t+1)
+    host = W.to_numpy({k: (None if v is None else v[..., :M * slabs]) for k, v in pristine.items()})
+    got = W.to_numpy({k: (None if v is None else v[..., :M * slabs]) for k, v in work.items()})   # last timed step's result
+
+    def slab(j):
+        return {k: (None if v is None else v[..., j * M:(j + 1) * M].copy()) for k, v in host.items()}   # (a copy: the oracle updates in place)
+
+    first = slab(0)
+    secs1, ost = time_oracle(wl, first, dt)                      # one core
+    refs = [slab(j) for j in range(slabs)]
+    t0 = time.perf_counter()
+    with ThreadPoolExecutor(max_workers=slabs) as ex:            # ctypes releases the GIL: real threads
+        list(ex.map(lambda r: time_oracle(wl, r, dt), refs))
+    secs_all = time.perf_counter() - t0
+    ref = {k: (None if host[k] is None else np.concatenate([r[k] for r in refs], axis=-1)) for k in host}
+    scale = dict(host)
+    if host.get("Srad") is not None:
+        scale["Erad"] = host["Erad"] + host["Srad"]
+    quasi = getattr(wl, "opacity_kind", 0) != 0 or getattr(wl, "spectrum", 0) != 0
+    afloor = afloor_quasi_newton(wl.newton_tol) if quasi else 1e-14      # tests/parity_util.py: why
+    res = compare(ref, got, scale, wl.c, wl.c_hat, afloor=afloor)
+    cpu = {"value": slabs * M * wl.Nq / secs_all, "unit": UNIT, "cores": slabs, "kind": "oracle",
+           "sample": f"first {slabs} x {M} cells of {workload_label(wl)}, one update each, one thread per core, dense LU",
+           "seconds": secs_all, "value_1core": M * wl.Nq / secs1, "seconds_1core": secs1, "host_cores_available": cores}
+    parity = {"cells": slabs * M, "tolerance": f"|d| <= 1e-10|ref| + {afloor:g} S_cell", "ok": all(v[0] == 0 for v in res.values()),
               "worst_excess_ratio": {k: v[1] for k, v in res.items()},
               "worst_relative_error_reported": {k: v[2] for k, v in res.items()},   # |d|/|ref| over |ref| > 1e-290, not gated
               "oracle_newton_evals_per_cell": ost["newton_evals_total"] / M}
@@ -420,11 +518,34 @@ def run_sustained(args) -> None:
     E1, P1 = torch.empty_like(E0), torch.empty_like(P0)
     resE = torch.zeros(calls, dtype=torch.float64, device="cuda")
     resP = torch.zeros(calls, dtype=torch.float64, device="cuda")
+    M, slabs, _ = cpu_sample_plan(args, wl)
+    keep0 = {k: (None if v is None else v[..., :M * slabs].clone()) for k, v in st.items()}     # U^(t) of call 0
+    keep1 = None
+
+    def counted_flops(dt_i):
+        """Algorithmic flops of the update this state is about to get: instrumented pass on a clone, untimed."""
+        clone = W.clone_state(st)
+        ctx.set_flop_counting(True)
+        ctx.reset_stats()
+        ctx.source_update(clone, dt_i, wl.c, wl.c_hat)
+        f = float(ctx.get_stats()["flops"])
+        ctx.set_flop_counting(False)
+        ctx.reset_stats()
+        del clone
+        return f
+
+    flops_first = counted_flops(wl.dt_of_call(0))
+    flops_last = 0.0
     sampler = ClockSampler(0)
     sampler.start()
     evs, launches0 = [], ctx.launch_count()
     for i in range(calls):
         dt = wl.dt_of_call(i)
+        if i == calls - 1 and calls > 1:
+            torch.cuda.synchronize()
+            st_stats = ctx.get_stats()
+            flops_last = counted_flops(dt)
+            launches0 += 1
         ctx.conserved_totals(st, wl.c, wl.c_hat, E0, P0)
         Es = st["Egas"].abs() + (wl.c / wl.c_hat) * st["Erad"].abs().sum(0)
         Ps = st["mom"].pow(2).sum(0).sqrt() + st["Frad"].pow(2).sum(0).sqrt().sum(0) / (wl.c * wl.c_hat)
@@ -433,6 +554,8 @@ def run_sustained(args) -> None:
         ctx.source_update(st, dt, wl.c, wl.c_hat)
         e1.record(stream)
         evs.append((e0, e1))
+        if i == 0:
+            keep1 = {k: (None if v is None else v[..., :M * slabs].clone()) for k, v in st.items()}
         ctx.conserved_totals(st, wl.c, wl.c_hat, E1, P1)
         resE[i] = ((E1 - E0).abs() / Es).max()
         dP = (P1 - P0).pow(2).sum(0).sqrt()
@@ -442,14 +565,29 @@ def run_sustained(args) -> None:
     clocks = sampler.stop()
     ms = [a.elapsed_time(b) for a, b in evs]
     stats = ctx.get_stats()
+    if calls > 1:                              # (the statistics were reset around the instrumented pass of the last call)
+        for k in ("newton_evals_total", "outer_trips_total", "n_newton_unconverged", "n_outer_unconverged"):
+            stats[k] += st_stats[k]
     total_s = sum(ms) * 1e-3
+    dfma = binding.measure_dfma_peak(1 << 22)
+    peak_tflops = 2.0 * dfma / 1e12
+    fl = flops_last if calls > 1 else flops_first
+    roofline = {"bound": "alu", "achieved": fl / (ms[-1] * 1e-3) / 1e12, "peak": peak_tflops, "unit": "TFLOP/s",
+                "frac": fl / (ms[-1] * 1e-3) / 1e12 / peak_tflops, "traffic": None,
+                "peak_source": "FP64 FMA rate measured in this run by mgrhd_measure_dfma_peak (x2 flop/FMA)",
+                "which_call": "last call (iteration counts fall from call to call); first call alongside",
+                "first_call": {"algorithmic_flops_per_cell_group": flops_first / (n * Nq),
+                               "frac": flops_first / (ms[0] * 1e-3) / 1e12 / peak_tflops},
+                "algorithmic_flops_per_cell_group": fl / (n * Nq)}
+    cpu, parity = run_cpu_baseline(args, wl, keep0, keep1, wl.dt_of_call(0))
     line = {
         "metric": METRIC, "value": n * Nq * calls / total_s, "unit": UNIT, "n_gpus": 1, "steps": calls, "warmup": 0,
         "ms_per_step": 1e3 * total_s / calls, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "config": {"workload": workload_label(wl) + " (sustained: successive calls, no restore)", "cells_per_gpu": n,
                    "Nq": Nq, "c": wl.c, "c_hat": wl.c_hat, "l2": "state larger than L2"},
-        "clocks": clocks, "gpu_launches": (ctx.launch_count() - launches0 - 2 * calls),
+        "clocks": clocks, "gpu_launches": (ctx.launch_count() - launches0 - 2 * calls), "roofline": roofline,
+        "cpu_baseline": cpu, "parity_sample": dict(parity, which="call 0"),
         "call_ms": {"first": ms[0], "min": min(ms), "max": max(ms), "last": ms[-1]},
         "iterations": {"newton_evals_per_cell_call": stats["newton_evals_total"] / (n * calls),
                        "outer_trips_per_cell_call": stats["outer_trips_total"] / (n * calls),
@@ -463,8 +601,23 @@ def run_sustained(args) -> None:
     print(json.dumps(line))
 
 
+def spawn_ranks(args) -> int:
+    """`python bench.py --gpus N` without a launcher: start the N ranks ourselves, exactly as the driver does."""
+    import socket
+    import subprocess
+
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
+
+
 def main():
     args = parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.impl == "ours" and args.sustained == 0:
+        raise SystemExit(spawn_ranks(args))
     if args.impl == "reference":
         run_reference(args)
     elif args.sustained > 0:
