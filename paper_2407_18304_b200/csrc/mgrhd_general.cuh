@@ -29,8 +29,8 @@ __device__ __forceinline__ double warp_sum(double v) {
   return v;
 }
 
-// [ (r^q - 1)/q ] of Eq. 30, ln r at q ln r = 0.
-__device__ __forceinline__ double eq30_bracket(double q, double lnr) {
+// [ (r^q - 1)/q ] of Eq. 30, ln r at q ln r = 0.  Out of line: four uses per group.
+__device__ __noinline__ double eq30_bracket(double q, double lnr) {
   const double z = q * lnr;
   return z == 0.0 ? lnr : expm1(z) / q;
 }
@@ -163,15 +163,21 @@ source_update_general_kernel(const __grid_constant__ Params P, const __grid_cons
         const double beta = P.h_over_k / T;
         // a1: edge functions at the lane's upper edges; the lower edge comes from the left, edge 0 from an
         // evaluation of its own (lane 0)
+        // (through the one out-of-line copy of the three branches: this kernel is bound by instruction fetch --
+        // its loop body exceeds the 32 KB the SM's instruction cache holds -- so code size comes first)
         double hy[GPL], hx[GPL], ly[GPL], lx[GPL];
         bool hs[GPL], ls[GPL];
-        int fl;
-#pragma unroll
-        for (int k = 0; k < GPL; ++k)
-          planck_edge_w(vg[k] ? nu_hi[k] * beta : NaN, 0, hy[k], hx[k], hs[k], fl);
+#pragma unroll 1
+        for (int k = 0; k < GPL; ++k) {
+          const EdgeOut o = planck_edge_call(vg[k] ? nu_hi[k] * beta : NaN);
+          hy[k] = o.yz; hx[k] = o.xi; hs[k] = o.small != 0;
+        }
         double e0y, e0x;
         bool e0s;
-        planck_edge_w(lane == 0 ? P.nu[0] * beta : NaN, 0, e0y, e0x, e0s, fl);
+        {
+          const EdgeOut o = planck_edge_call(lane == 0 ? P.nu[0] * beta : NaN);
+          e0y = o.yz; e0x = o.xi; e0s = o.small != 0;
+        }
         {
           const double uy = __shfl_up_sync(FULL, hy[GPL - 1], 1), ux = __shfl_up_sync(FULL, hx[GPL - 1], 1);
           const int us = __shfl_up_sync(FULL, (int)hs[GPL - 1], 1);

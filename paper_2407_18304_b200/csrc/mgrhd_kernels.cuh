@@ -320,7 +320,7 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
       const double aT4 = P.a_rad * T2 * T2;
       const double beta = P.h_over_k * invT;
       if (KT) {                                         // opacities at this trial temperature
-        const double f = pow(T * P.inv_T_ref, P.p_T);
+        const double f = exp(P.p_T * log(T * P.inv_T_ref));   // (pow() inlines ~3 KB more code: instruction cache)
         if (ev) { chis = chis0 * f; inv_chis = inv_chis0 / f; }
       }
       const double itau_c = inv_chis * inv_cdt;         // 1/(c_hat dt chi_E,g) = itau_c * inv_k_mean[g]
