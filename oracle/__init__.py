@@ -10,6 +10,8 @@ from .oracle import (  # noqa: F401
     chi_flux,
     chi_mean,
     free_slopes,
+    imex_step_1d,
+    transport_add,
     arrowhead_solve,
     lu_solve,
     planck_dY,

@@ -581,3 +581,115 @@ int oracle_source_update(const oracle_model* m, long long n, const double* rho,
 }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------------------
+// L4 (round 2): explicit radiation transport in 1-D and the two-stage
+// IMEX step around the source update (Eq. 33-36).  TEST INFRASTRUCTURE.
+//
+// Eq. 34: dE_g/dt = -(c_hat/c) dF_g^x/dx,  dF_g^i/dt = -c c_hat dP_g^{xi}/dx  (1-D, x only), gas fields
+// have no transport term.  The paper defers the spatial discretisation to "Paper II";
+// the reading used by BOTH implementations (S22) is the plainest conservative one: piecewise
+// constant states, local Lax-Friedrichs interface fluxes with the signal speed c_hat,
+//   f_{i+1/2} = (f(u_i) + f(u_{i+1}))/2 - (c_hat/2)(u_{i+1} - u_i),
+//   u = (E_g, F_g^x, F_g^y, F_g^z),  f(u) = ((c_hat/c) F^x, c c_hat P^{xx}, c c_hat P^{xy}, c c_hat P^{xz}),
+// P_g from the closure of reading S7 (M1 or Eddington), periodic (bc = 0) or zero-gradient (bc = 1) ends.
+// For a beam (|F| = cE along x) this is exact upwinding.  Parity unpinned beyond: conservation, the
+// upwind closed form, uniform states, and the stage equations of Eq. 35-36 checked with the brute-force
+// residual (tests/test_oracle_transport.py).
+// ---------------------------------------------------------------------------
+namespace {
+
+// P^{x i} (i = x, y, z) of one group from (E, F): reading S7.
+void pressure_x(int closure, double E, const double F[3], double c, double Px[3]) {
+  double Fn = std::sqrt(F[0] * F[0] + F[1] * F[1] + F[2] * F[2]);
+  if (closure == 1 || !(E > 0.0) || Fn == 0.0) {
+    Px[0] = E / 3.0; Px[1] = 0.0; Px[2] = 0.0;
+    return;
+  }
+  double f = Fn / (c * E);
+  if (f > 1.0) f = 1.0;
+  double chi = (3.0 + 4.0 * f * f) / (5.0 + 2.0 * std::sqrt(4.0 - 3.0 * f * f));
+  double n[3] = {F[0] / Fn, F[1] / Fn, F[2] / Fn};
+  for (int i = 0; i < 3; ++i) Px[i] = E * (0.5 * (3.0 * chi - 1.0) * n[0] * n[i]);
+  Px[0] += E * 0.5 * (1.0 - chi);
+}
+
+}  // namespace
+
+extern "C" {
+
+// dst += wdt * T(src) for E_g and F_g of every group; nx cells along x (cell index fastest), spacing dx.
+// src and dst may not alias.  Arrays as in oracle_source_update ([Nq][nx]).
+int oracle_transport_add(int Nq, int closure, long long nx, double dx, double wdt, double c, double chat, int bc,
+                         const double* sE, const double* sF0, const double* sF1, const double* sF2,
+                         double* dE, double* dF0, double* dF1, double* dF2) {
+  if (Nq < 1 || nx < 1 || !(dx > 0.0) || !(c > 0.0) || !(chat > 0.0) || bc < 0 || bc > 1) return -1;
+  std::vector<double> flux((size_t)(nx + 1) * 4);   // interface i-1/2 at index i, i = 0..nx
+  for (int g = 0; g < Nq; ++g) {
+    const double* E = sE + (size_t)g * nx;
+    const double* Fs[3] = {sF0 + (size_t)g * nx, sF1 + (size_t)g * nx, sF2 + (size_t)g * nx};
+    auto cellidx = [&](long long i) -> long long {
+      if (bc == 0) return (i % nx + nx) % nx;
+      return i < 0 ? 0 : (i >= nx ? nx - 1 : i);
+    };
+    for (long long i = 0; i <= nx; ++i) {
+      const long long a = cellidx(i - 1), b = cellidx(i);
+      double Fa[3] = {Fs[0][a], Fs[1][a], Fs[2][a]}, Fb[3] = {Fs[0][b], Fs[1][b], Fs[2][b]}, Pa[3], Pb[3];
+      pressure_x(closure, E[a], Fa, c, Pa);
+      pressure_x(closure, E[b], Fb, c, Pb);
+      double* f = &flux[(size_t)i * 4];
+      f[0] = 0.5 * ((chat / c) * Fa[0] + (chat / c) * Fb[0]) - 0.5 * chat * (E[b] - E[a]);
+      for (int k = 0; k < 3; ++k) f[1 + k] = 0.5 * (c * chat * Pa[k] + c * chat * Pb[k]) - 0.5 * chat * (Fb[k] - Fa[k]);
+    }
+    double* out[4] = {dE + (size_t)g * nx, dF0 + (size_t)g * nx, dF1 + (size_t)g * nx, dF2 + (size_t)g * nx};
+    for (long long i = 0; i < nx; ++i)
+      for (int k = 0; k < 4; ++k) out[k][i] += -(wdt / dx) * (flux[(size_t)(i + 1) * 4 + k] - flux[(size_t)i * 4 + k]);
+  }
+  return 0;
+}
+
+// One IMEX step of Eq. 35-36 in 1-D, in place (U^n -> U^(n+1)); Srad is not supported here (NULL).
+//   stage 1: U* = U^n + dt T(U^n);  U^(n+1/2) = U* + dt S(U^(n+1/2))          (source update with theta = 1)
+//   stage 2: U** = U^n + dt [T(U^n)/2 + T(U^(n+1/2))/2] + (dt/2) S(U^(n+1/2)) = (U^n + U^(n+1/2))/2 + (dt/2) T(U^(n+1/2))
+//            (since dt S(U^(n+1/2)) = U^(n+1/2) - U* and dt T(U^n) = U* - U^n);  U^(n+1) = U** + (dt/2) S(U^(n+1))   (theta = 1/2)
+int oracle_imex_step_1d(const oracle_model* m, long long nx, double dx, double dt, double c, double chat, int bc,
+                        const double* rho, double* mom0, double* mom1, double* mom2, double* Egas, double* Erad,
+                        double* Frad0, double* Frad1, double* Frad2, const double* kappa_scale, oracle_stats* stats) {
+  if (!m) return -1;
+  const size_t n = (size_t)nx, ng = (size_t)m->Nq * n;
+  std::vector<double> w_m0(mom0, mom0 + n), w_m1(mom1, mom1 + n), w_m2(mom2, mom2 + n), w_eg(Egas, Egas + n),
+      w_E(Erad, Erad + ng), w_F0(Frad0, Frad0 + ng), w_F1(Frad1, Frad1 + ng), w_F2(Frad2, Frad2 + ng);
+  // stage 1
+  int rc = oracle_transport_add(m->Nq, m->closure, nx, dx, dt, c, chat, bc, Erad, Frad0, Frad1, Frad2,
+                                w_E.data(), w_F0.data(), w_F1.data(), w_F2.data());
+  if (rc) return rc;
+  oracle_stats s1, s2;
+  rc = oracle_source_update(m, nx, rho, w_m0.data(), w_m1.data(), w_m2.data(), w_eg.data(), w_E.data(), w_F0.data(),
+                            w_F1.data(), w_F2.data(), kappa_scale, nullptr, dt, c, chat, &s1);
+  if (rc) return rc;
+  // stage 2
+  for (size_t i = 0; i < n; ++i) {
+    mom0[i] = 0.5 * (mom0[i] + w_m0[i]); mom1[i] = 0.5 * (mom1[i] + w_m1[i]); mom2[i] = 0.5 * (mom2[i] + w_m2[i]);
+    Egas[i] = 0.5 * (Egas[i] + w_eg[i]);
+  }
+  for (size_t i = 0; i < ng; ++i) {
+    Erad[i] = 0.5 * (Erad[i] + w_E[i]);
+    Frad0[i] = 0.5 * (Frad0[i] + w_F0[i]); Frad1[i] = 0.5 * (Frad1[i] + w_F1[i]); Frad2[i] = 0.5 * (Frad2[i] + w_F2[i]);
+  }
+  rc = oracle_transport_add(m->Nq, m->closure, nx, dx, 0.5 * dt, c, chat, bc, w_E.data(), w_F0.data(), w_F1.data(),
+                            w_F2.data(), Erad, Frad0, Frad1, Frad2);
+  if (rc) return rc;
+  rc = oracle_source_update(m, nx, rho, mom0, mom1, mom2, Egas, Erad, Frad0, Frad1, Frad2, kappa_scale, nullptr,
+                            0.5 * dt, c, chat, &s2);
+  if (stats) {
+    *stats = s2;
+    stats->newton_evals_total += s1.newton_evals_total;
+    stats->outer_trips_total += s1.outer_trips_total;
+    stats->n_newton_unconverged += s1.n_newton_unconverged;
+    stats->n_outer_unconverged += s1.n_outer_unconverged;
+    stats->n_T_nonpositive_steps += s1.n_T_nonpositive_steps;
+  }
+  return rc;
+}
+
+}  // extern "C"

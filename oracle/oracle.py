@@ -97,6 +97,11 @@ def _load():
         L.oracle_source_update.argtypes = (
             [ctypes.POINTER(_CModel), ctypes.c_longlong] + [dp] * 11 + [d, d, d, ctypes.POINTER(_CStats)]
         )
+        L.oracle_transport_add.restype = ctypes.c_int
+        L.oracle_transport_add.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_longlong, d, d, d, d, ctypes.c_int] + [dp] * 8
+        L.oracle_imex_step_1d.restype = ctypes.c_int
+        L.oracle_imex_step_1d.argtypes = ([ctypes.POINTER(_CModel), ctypes.c_longlong, d, d, d, d, ctypes.c_int] + [dp] * 10
+                                          + [ctypes.POINTER(_CStats)])
         L.oracle_free_slopes.restype = None
         L.oracle_free_slopes.argtypes = [ctypes.c_int, dp, dp, dp]
         _lib = L
@@ -249,3 +254,31 @@ def source_update(model: OracleModel, state: dict, dt: float, c: float, c_hat: f
     out["newton_hist"] = np.array(st.newton_hist[:], dtype=np.int64)
     out["outer_hist"] = np.array(st.outer_hist[:], dtype=np.int64)
     return out
+
+
+def transport_add(src: dict, dst: dict, closure: int, dx: float, wdt: float, c: float, c_hat: float, bc: int = 0) -> None:
+    """dst[Erad, Frad] += wdt * T(src) (Eq. 34 in 1-D, reading S22); src, dst: state dicts ([Nq, nx] arrays)."""
+    Nq, nx = src["Erad"].shape
+    for st in (src, dst):
+        assert st["Erad"].flags.c_contiguous and st["Frad"].flags.c_contiguous
+    rc = _load().oracle_transport_add(Nq, closure, nx, float(dx), float(wdt), float(c), float(c_hat), bc,
+                                      _p(src["Erad"]), _p(src["Frad"][0]), _p(src["Frad"][1]), _p(src["Frad"][2]),
+                                      _p(dst["Erad"]), _p(dst["Frad"][0]), _p(dst["Frad"][1]), _p(dst["Frad"][2]))
+    if rc != 0:
+        raise ValueError(f"oracle_transport_add: argument error {rc}")
+
+
+def imex_step_1d(model: OracleModel, state: dict, dx: float, dt: float, c: float, c_hat: float, bc: int = 0) -> dict:
+    """One two-stage IMEX step (Eq. 35-36) of a 1-D state, in place.  Returns the summed source-update stats."""
+    cm = model._c()
+    nx = state["rho"].shape[0]
+    ks = state.get("kappa_scale")
+    st = _CStats()
+    rc = _load().oracle_imex_step_1d(
+        ctypes.byref(cm), nx, float(dx), float(dt), float(c), float(c_hat), bc, _p(state["rho"]),
+        _p(state["mom"][0]), _p(state["mom"][1]), _p(state["mom"][2]), _p(state["Egas"]), _p(state["Erad"]),
+        _p(state["Frad"][0]), _p(state["Frad"][1]), _p(state["Frad"][2]), _p(ks) if ks is not None else None,
+        ctypes.byref(st))
+    if rc != 0:
+        raise ValueError(f"oracle_imex_step_1d: argument error {rc}")
+    return {k: getattr(st, k) for k, _ in _CStats._fields_ if not k.endswith("_hist")}
