@@ -137,6 +137,25 @@ int mgrhd_source_update(mgrhd_ctx *ctx, const mgrhd_state *state_dev, long long 
 int mgrhd_source_update_host(mgrhd_ctx *ctx, const mgrhd_state *state_host, long long ncells,
                              double dt, double c, double c_hat);
 
+/* Explicit radiation transport of Eq. 34 in one dimension:
+ *   dst.E_g += w_dt * [-(c_hat/c) dF_g^x/dx](src),   dst.F_g^i += w_dt * [-c c_hat dP_g^{xi}/dx](src)
+ * for the nx cells of a row (cell index = position along x, spacing dx), every group; the gas fields have no
+ * transport term.  The paper defers the discretisation to Paper II: here piecewise-constant states and local
+ * Lax-Friedrichs interface fluxes with the signal speed c_hat, P_g from the context's closure (S22).
+ * bc: 0 periodic, 1 zero-gradient.  src and dst are DEVICE states that must not alias; only Erad and Frad of
+ * dst are touched.  Stream-ordered, asynchronous, one kernel. */
+int mgrhd_transport_add(mgrhd_ctx *ctx, const mgrhd_state *src_dev, const mgrhd_state *dst_dev, long long nx,
+                        double dx, double w_dt, double c, double c_hat, int bc, void *cuda_stream);
+
+/* One two-stage IMEX step of Eq. 35-36 of a 1-D row, in place in U_dev (U^n -> U^(n+1)):
+ *   stage 1: U* = U^n + dt T(U^n);  U^(n+1/2) = U* + dt S(U^(n+1/2))       (mgrhd_source_update, theta = 1)
+ *   stage 2: U** = U^n + dt [T(U^n) + T(U^(n+1/2))]/2 + (dt/2) S(U^(n+1/2)); U^(n+1) = U** + (dt/2) S(U^(n+1)) (theta = 1/2)
+ * work_dev: a caller-owned DEVICE scratch state of the same shape (its mom, Egas, Erad, Frad are overwritten; its
+ * rho, kappa_scale, Srad are ignored).  U_dev->Srad must be NULL.  Stream-ordered, asynchronous: 8 copies, two
+ * transport kernels, 8 averaging kernels and two source updates are enqueued. */
+int mgrhd_imex_step_1d(mgrhd_ctx *ctx, const mgrhd_state *U_dev, const mgrhd_state *work_dev, long long nx,
+                       double dx, double dt, double c, double c_hat, int bc, void *cuda_stream);
+
 /* Per-cell conserved totals of a DEVICE state, for conservation checks:
  *   out_energy[n]      = E_gas + (c/c_hat) sum_g E_g
  *   out_momentum[3][n] = rho v^i + (c c_hat)^-1 sum_g F_g^i

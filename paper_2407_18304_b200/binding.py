@@ -19,6 +19,7 @@ HIST = 64
 
 EXPORTS = (
     "mgrhd_init", "mgrhd_source_update", "mgrhd_source_update_host", "mgrhd_conserved_totals",
+    "mgrhd_transport_add", "mgrhd_imex_step_1d",
     "mgrhd_get_stats", "mgrhd_reset_stats", "mgrhd_set_flop_counting", "mgrhd_launch_count", "mgrhd_planck_edge_functions", "mgrhd_measure_dfma_peak",
     "mgrhd_last_error", "mgrhd_free",
 )
@@ -76,6 +77,10 @@ def load_library() -> ctypes.CDLL:
     L.mgrhd_source_update.argtypes = [vp, ctypes.POINTER(State), ll, d, d, d, vp]
     L.mgrhd_source_update_host.restype = i
     L.mgrhd_source_update_host.argtypes = [vp, ctypes.POINTER(State), ll, d, d, d]
+    L.mgrhd_transport_add.restype = i
+    L.mgrhd_transport_add.argtypes = [vp, ctypes.POINTER(State), ctypes.POINTER(State), ll, d, d, d, d, i, vp]
+    L.mgrhd_imex_step_1d.restype = i
+    L.mgrhd_imex_step_1d.argtypes = [vp, ctypes.POINTER(State), ctypes.POINTER(State), ll, d, d, d, d, i, vp]
     L.mgrhd_conserved_totals.restype = i
     L.mgrhd_conserved_totals.argtypes = [vp, ctypes.POINTER(State), ll, d, d, vp, vp, vp]
     L.mgrhd_get_stats.restype = i
@@ -197,6 +202,28 @@ class Context:
         s = _state_struct(state, self.Nq, n)
         _check(self._L.mgrhd_source_update_host(self._h, ctypes.byref(s), n, dt, c, c_hat),
                "mgrhd_source_update_host")
+
+    def transport_add(self, src: dict, dst: dict, dx: float, w_dt: float, c: float, c_hat: float, bc: int = 0,
+                      stream=None) -> None:
+        """mgrhd_transport_add: dst[Erad, Frad] += w_dt * T(src) along a 1-D row of DEVICE tensors."""
+        n = int(src["rho"].shape[0])
+        if stream is None:
+            import torch
+            stream = torch.cuda.current_stream().cuda_stream
+        a, b = _state_struct(src, self.Nq, n), _state_struct(dst, self.Nq, n)
+        _check(self._L.mgrhd_transport_add(self._h, ctypes.byref(a), ctypes.byref(b), n, dx, w_dt, c, c_hat, bc,
+                                           ctypes.c_void_p(stream)), "mgrhd_transport_add")
+
+    def imex_step_1d(self, state: dict, work: dict, dx: float, dt: float, c: float, c_hat: float, bc: int = 0,
+                     stream=None) -> None:
+        """mgrhd_imex_step_1d: one two-stage IMEX step (Eq. 35-36) of a 1-D row, in place; `work` is scratch."""
+        n = int(state["rho"].shape[0])
+        if stream is None:
+            import torch
+            stream = torch.cuda.current_stream().cuda_stream
+        a, b = _state_struct(state, self.Nq, n), _state_struct(work, self.Nq, n)
+        _check(self._L.mgrhd_imex_step_1d(self._h, ctypes.byref(a), ctypes.byref(b), n, dx, dt, c, c_hat, bc,
+                                          ctypes.c_void_p(stream)), "mgrhd_imex_step_1d")
 
     def conserved_totals(self, state: dict, c: float, c_hat: float, out_energy, out_momentum, stream=None) -> None:
         n = int(state["rho"].shape[0])

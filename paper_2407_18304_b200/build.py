@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmgrhd.so")
 SOURCES = ["mgrhd_api.cu"]
-DEPS = ["mgrhd_api.cu", "mgrhd_kernels.cuh", "mgrhd_general.cuh", "mgrhd_planck.cuh", "mgrhd_params.h",
+DEPS = ["mgrhd_api.cu", "mgrhd_kernels.cuh", "mgrhd_general.cuh", "mgrhd_transport.cuh", "mgrhd_planck.cuh", "mgrhd_params.h",
         os.path.join("..", "..", "include", "mgrhd.h")]
 
 NVCC_FLAGS = [

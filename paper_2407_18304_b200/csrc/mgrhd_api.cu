@@ -12,6 +12,7 @@
 #include <new>
 
 #include "mgrhd_general.cuh"
+#include "mgrhd_transport.cuh"
 
 using namespace mgrhd;
 
@@ -472,6 +473,76 @@ int mgrhd_source_update_host(mgrhd_ctx* ctx, const mgrhd_state* s, long long n, 
   }
   for (int k = 0; k < kSlabs; ++k) CU(cudaStreamSynchronize(ctx->slab_stream[k]));
   return MGRHD_OK;
+}
+
+static int launch_transport(mgrhd_ctx* ctx, const StatePtrs& src, const StatePtrs& dst, long long nx, double dx,
+                            double wdt, double c, double chat, int bc, cudaStream_t st) {
+  const long long tiles = (nx + kTransportTile - 3) / (kTransportTile - 2);
+  dim3 grid((unsigned)tiles, (unsigned)ctx->P.Nq);
+  transport_add_kernel<<<grid, kTransportTile, 0, st>>>(src, dst, ctx->P.closure, nx, nx, nx, wdt / dx, c, chat, bc);
+  ctx->launches++;
+  ctx->last_stream = st;
+  CU(cudaGetLastError());
+  return MGRHD_OK;
+}
+
+static int check_transport(const mgrhd_ctx* ctx, const mgrhd_state* a, const mgrhd_state* b, long long nx, double dx,
+                           double c, double chat, int bc) {
+  int rc = check_call(ctx, a, nx, 1.0, c, chat);
+  if (rc != MGRHD_OK) return rc;
+  if (!b || bc < 0 || bc > 1) return MGRHD_ERR_ARG;
+  if (!(dx > 0.0)) return MGRHD_ERR_RANGE;
+  if (nx > 0 && (!b->Erad || !b->Frad[0] || !b->Frad[1] || !b->Frad[2])) return MGRHD_ERR_ARG;
+  if (nx > 0 && (a->Erad == b->Erad || a->Frad[0] == b->Frad[0])) return MGRHD_ERR_ARG;      // no aliasing
+  if (nx > 0 && nx > (1ll << 31) * (kTransportTile - 2)) return MGRHD_ERR_ARG;
+  return MGRHD_OK;
+}
+
+int mgrhd_transport_add(mgrhd_ctx* ctx, const mgrhd_state* src, const mgrhd_state* dst, long long nx, double dx,
+                        double w_dt, double c, double chat, int bc, void* stream) {
+  int rc = check_transport(ctx, src, dst, nx, dx, c, chat, bc);
+  if (rc != MGRHD_OK) return rc;
+  if (!std::isfinite(w_dt)) return MGRHD_ERR_RANGE;
+  if (nx == 0) return MGRHD_OK;
+  return launch_transport(ctx, to_ptrs(src), to_ptrs(dst), nx, dx, w_dt, c, chat, bc, (cudaStream_t)stream);
+}
+
+int mgrhd_imex_step_1d(mgrhd_ctx* ctx, const mgrhd_state* U, const mgrhd_state* W, long long nx, double dx, double dt,
+                       double c, double chat, int bc, void* stream) {
+  int rc = check_transport(ctx, U, W, nx, dx, c, chat, bc);
+  if (rc != MGRHD_OK) return rc;
+  if (!(dt > 0.0)) return MGRHD_ERR_RANGE;
+  if (U->Srad) return MGRHD_ERR_ARG;                      // a per-update source has no place in the two stages
+  if (nx > 0 && (!W->mom[0] || !W->mom[1] || !W->mom[2] || !W->Egas)) return MGRHD_ERR_ARG;
+  if (nx == 0) return MGRHD_OK;
+  cudaStream_t st = (cudaStream_t)stream;
+  const int Nq = ctx->P.Nq;
+  const size_t b1 = (size_t)nx * sizeof(double), bq = b1 * Nq;
+  StatePtrs SU = to_ptrs(U), SW = to_ptrs(W);
+  SW.rho = SU.rho;                                        // the work state borrows the read-only fields
+  SW.kappa_scale = SU.kappa_scale;
+  SW.Srad = nullptr;
+  // stage 1 (Eq. 35): W = U^n + dt T(U^n), then the implicit source update with theta = 1
+  for (int i = 0; i < 3; ++i) CU(cudaMemcpyAsync(SW.mom[i], SU.mom[i], b1, cudaMemcpyDeviceToDevice, st));
+  CU(cudaMemcpyAsync(SW.Egas, SU.Egas, b1, cudaMemcpyDeviceToDevice, st));
+  CU(cudaMemcpyAsync(SW.Erad, SU.Erad, bq, cudaMemcpyDeviceToDevice, st));
+  for (int i = 0; i < 3; ++i) CU(cudaMemcpyAsync(SW.Frad[i], SU.Frad[i], bq, cudaMemcpyDeviceToDevice, st));
+  rc = launch_transport(ctx, SU, SW, nx, dx, dt, c, chat, bc, st);
+  if (rc != MGRHD_OK) return rc;
+  rc = launch_update(ctx, SW, nx, nx, dt, c, chat, st, ctx->scratch);
+  if (rc != MGRHD_OK) return rc;
+  // stage 2 (Eq. 36): U = (U^n + U^(n+1/2))/2 + (dt/2) T(U^(n+1/2)), then the source update with theta = 1/2
+  // (dt S(U^(n+1/2)) = U^(n+1/2) - U* and dt T(U^n) = U* - U^n turn Eq. 36's explicit part into this form)
+  const int ab = ctx->sm_count * 8;
+  for (int i = 0; i < 3; ++i) average_kernel<<<ab, 256, 0, st>>>(SU.mom[i], SW.mom[i], nx);
+  average_kernel<<<ab, 256, 0, st>>>(SU.Egas, SW.Egas, nx);
+  average_kernel<<<ab, 256, 0, st>>>(SU.Erad, SW.Erad, nx * Nq);
+  for (int i = 0; i < 3; ++i) average_kernel<<<ab, 256, 0, st>>>(SU.Frad[i], SW.Frad[i], nx * Nq);
+  ctx->launches += 8;
+  CU(cudaGetLastError());
+  rc = launch_transport(ctx, SW, SU, nx, dx, 0.5 * dt, c, chat, bc, st);
+  if (rc != MGRHD_OK) return rc;
+  return launch_update(ctx, SU, nx, nx, 0.5 * dt, c, chat, st, ctx->scratch);
 }
 
 int mgrhd_get_stats(mgrhd_ctx* ctx, mgrhd_stats* out) {

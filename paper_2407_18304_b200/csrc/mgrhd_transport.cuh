@@ -1,0 +1,89 @@
+// mgrhd_transport.cuh -- explicit radiation transport T(U) of Eq. 34 in 1-D and the
+// element-wise helper of the two-stage IMEX step (Eq. 35-36).  SURVEY 8(f) NEXT-3.
+//
+//   dE_g/dt = -(c_hat/c) dF_g^x/dx,   dF_g^i/dt = -c c_hat dP_g^{xi}/dx,   gas fields: no transport term.
+//
+// The paper defers the spatial discretisation to Paper II; the reading used here and in the oracle
+// (S22) is piecewise-constant states with local Lax-Friedrichs interface fluxes at the signal
+// speed c_hat:  f_{i+1/2} = (f(u_i) + f(u_{i+1}))/2 - (c_hat/2)(u_{i+1} - u_i),  u = (E, F^x, F^y, F^z),
+// f(u) = ((c_hat/c) F^x, c c_hat P^xx, c c_hat P^xy, c c_hat P^xz), P from the closure of reading S7.
+//
+// HBM-bound: per cell-group the kernel reads u of the source state (4 doubles; the two halo cells of a tile
+// are re-read from L2), reads and writes u of the destination (4 + 4): 96 algorithmic bytes.  One thread per
+// (group, cell): f(u_i) is formed once per cell (one closure: one sqrt, two divisions), staged with u_i in
+// shared memory, and each interior thread of the tile combines its two interfaces.  Tiles of 256 cells
+// overlap by two, so 254/256 of the threads produce output; the cell index is the fastest in memory, so every
+// load and store of a warp is one contiguous 256-byte run.
+//
+// Product code; shares nothing with oracle/.
+#pragma once
+#include "mgrhd_params.h"
+
+namespace mgrhd {
+
+constexpr int kTransportTile = 256;
+
+// P^{x i} c c_hat and (c_hat/c) F^x of one cell-group: the flux vector f(u).
+__device__ __forceinline__ void transport_flux(int closure, double E, double F0, double F1, double F2, double c,
+                                               double chat, double (&f)[4]) {
+  const double Fn = sqrt(F0 * F0 + F1 * F1 + F2 * F2);
+  double Pxx = E / 3.0, Pxy = 0.0, Pxz = 0.0;
+  if (!(closure == 1 || !(E > 0.0) || Fn == 0.0)) {
+    double ff = Fn / (c * E);
+    if (ff > 1.0) ff = 1.0;
+    const double chi = (3.0 + 4.0 * ff * ff) / (5.0 + 2.0 * sqrt(4.0 - 3.0 * ff * ff));   // Levermore 1984
+    const double n0 = F0 / Fn, n1 = F1 / Fn, n2 = F2 / Fn;
+    const double an = E * (0.5 * (3.0 * chi - 1.0));
+    Pxx = an * n0 * n0 + E * 0.5 * (1.0 - chi);
+    Pxy = an * n0 * n1;
+    Pxz = an * n0 * n2;
+  }
+  f[0] = (chat / c) * F0;
+  f[1] = c * chat * Pxx;
+  f[2] = c * chat * Pxy;
+  f[3] = c * chat * Pxz;
+}
+
+// dst(E_g, F_g) += wdt * T(src) for nx cells; grid = (ceil(nx / (tile - 2)), Nq), block = tile threads.
+// bc: 0 periodic, 1 zero-gradient.  src and dst must not alias.
+__global__ void __launch_bounds__(kTransportTile)
+transport_add_kernel(const __grid_constant__ StatePtrs src, const __grid_constant__ StatePtrs dst, int closure,
+                     long long nx, long long stride_src, long long stride_dst, double wdt_over_dx, double c,
+                     double chat, int bc) {
+  __shared__ double s_u[4][kTransportTile];
+  __shared__ double s_f[4][kTransportTile];
+  const int t = threadIdx.x;
+  const long long g = blockIdx.y;
+  const long long i = (long long)blockIdx.x * (kTransportTile - 2) + t - 1;     // cell of this thread (halo: i0 - 1, i0 + tile - 2)
+  long long j = i;                                                              // the cell it reads
+  if (bc == 0) j = (i % nx + nx) % nx;
+  else j = i < 0 ? 0 : (i >= nx ? nx - 1 : i);
+  const bool in_range = i <= nx;                                                // (cells beyond nx + 1 are never needed)
+  double u[4] = {0.0, 0.0, 0.0, 0.0}, f[4] = {0.0, 0.0, 0.0, 0.0};
+  if (in_range) {
+    const long long o = g * stride_src + j;
+    u[0] = src.Erad[o]; u[1] = src.Frad[0][o]; u[2] = src.Frad[1][o]; u[3] = src.Frad[2][o];
+    transport_flux(closure, u[0], u[1], u[2], u[3], c, chat, f);
+  }
+#pragma unroll
+  for (int k = 0; k < 4; ++k) { s_u[k][t] = u[k]; s_f[k][t] = f[k]; }
+  __syncthreads();
+  if (t >= 1 && t <= kTransportTile - 2 && i < nx) {
+    const long long o = g * stride_dst + i;
+    double* const out[4] = {dst.Erad, dst.Frad[0], dst.Frad[1], dst.Frad[2]};
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      const double fl = 0.5 * (s_f[k][t - 1] + s_f[k][t]) - 0.5 * chat * (s_u[k][t] - s_u[k][t - 1]);
+      const double fr = 0.5 * (s_f[k][t] + s_f[k][t + 1]) - 0.5 * chat * (s_u[k][t + 1] - s_u[k][t]);
+      out[k][o] += -wdt_over_dx * (fr - fl);
+    }
+  }
+}
+
+// a = (a + b)/2, element-wise (stage 2 of Eq. 36: (U^n + U^(n+1/2))/2).
+__global__ void average_kernel(double* __restrict__ a, const double* __restrict__ b, long long n) {
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)
+    a[i] = 0.5 * (a[i] + b[i]);
+}
+
+}  // namespace mgrhd
