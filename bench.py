@@ -42,6 +42,9 @@ def parse_args():
     ap.add_argument("--variant", default="default", choices=["default", "source", "ktemp", "free_slope", "edge_table"],
                     help="model option on top of the workload (SURVEY 8(f) rows): S_g present; kappa (T/T_ref)^1.5; "
                          "free-slope spectrum fit; edge opacities tabulated in T with alpha from Eq. 20")
+    ap.add_argument("--imex", action="store_true",
+                    help="SURVEY 8(f) NEXT-3: time the explicit 1-D transport kernel (HBM roofline) and whole two-stage "
+                         "IMEX steps (Eq. 35-36) on the workload read as one periodic row of cells")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -614,8 +617,78 @@ def spawn_ranks(args) -> int:
     return subprocess.call(cmd)
 
 
+def run_imex(args) -> None:
+    """The transport kernel by itself (HBM-bound: 96 algorithmic bytes per cell-group) and the IMEX step around it."""
+    import torch
+
+    from paper_2407_18304_b200 import binding, build, workloads as W
+
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    build.build()
+    wl = W.workload(args.workload, ncells=args.cells)
+    n, Nq = wl.ncells, wl.Nq
+    pristine = wl.make_state(device="cuda")
+    U, Wk = W.clone_state(pristine), W.clone_state(pristine)
+    ctx = binding.Context.from_workload(wl)
+    stream = torch.cuda.current_stream()
+    dx = 1.0
+    dt = 0.5 * dx / wl.c_hat                      # radiation CFL 0.5
+
+    def timed(fn, reps, warm):
+        for _ in range(warm):
+            fn()
+        torch.cuda.synchronize()
+        evs = []
+        for _ in range(reps):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream); fn(); e1.record(stream)
+            evs.append((e0, e1))
+        torch.cuda.synchronize()
+        return [a.elapsed_time(b) for a, b in evs]
+
+    sampler = ClockSampler(0)
+    sampler.start()
+    t_ms = timed(lambda: ctx.transport_add(pristine, Wk, dx, dt, wl.c, wl.c_hat, 0), max(args.steps, 5), max(args.warmup, 3))
+
+    def step():
+        copy_state(U, pristine)
+        ctx.imex_step_1d(U, Wk, dx, dt, wl.c, wl.c_hat, 0)
+
+    launches0 = ctx.launch_count()
+    s_ms = timed(step, args.steps, args.warmup)
+    gpu_launches = (ctx.launch_count() - launches0) * args.steps // (args.steps + args.warmup)
+    clocks = sampler.stop()
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        peaks = {}
+    hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
+    tb = 96.0 * n * Nq                            # read u of src (4), read + write u of dst (4 + 4) doubles per cell-group
+    t_avg = sum(t_ms) / len(t_ms) * 1e-3
+    restore_ms = timed(lambda: copy_state(U, pristine), 3, 1)
+    step_s = (sum(s_ms) / len(s_ms) - sum(restore_ms) / len(restore_ms)) * 1e-3
+    line = {
+        "metric": "IMEX-step cell-groups/sec (FP64; two transport sweeps + two implicit source updates, Eq. 35-36)",
+        "value": n * Nq / step_s, "unit": "cell-group steps/s", "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": 1e3 * step_s, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
+        "config": {"workload": workload_label(wl) + " as one periodic row (1-D)", "cells_per_gpu": n, "Nq": Nq,
+                   "radiation_cfl": 0.5, "l2": "state larger than L2" if state_nbytes(pristine) > (512 << 20) else "state near L2 size"},
+        "clocks": clocks, "gpu_launches": gpu_launches,
+        "roofline": {"kernel": "transport_add_kernel", "bound": "hbm", "achieved": tb / t_avg / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                     "frac": tb / t_avg / 1e9 / hbm_peak, "traffic": None, "algorithmic_bytes_per_cell_group": 96,
+                     "ms_per_launch": 1e3 * t_avg,
+                     "peak_source": "MEASURED_PEAKS.json hbm_gbs" if peaks else "fallback 6650 GB/s"},
+    }
+    ctx.free()
+    print(json.dumps(line))
+
+
 def main():
     args = parse_args()
+    if args.imex and args.impl == "ours":
+        return run_imex(args)
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.impl == "ours" and args.sustained == 0:
         raise SystemExit(spawn_ranks(args))
     if args.impl == "reference":
