@@ -61,7 +61,11 @@ typedef struct {
   int newton_maxit;        /* cap on Newton steps per outer trip (paper silent; 50)            */
   int outer_maxit;         /* cap on outer trips (paper silent; 50)                            */
   double outer_tol;        /* 1e-13 of PAPER.md:465                                            */
-  int outer_stop;          /* 0 = paper rule only; 1 = also |dF_g|<=rel*|F_g|, |d rho v|<=rel*|rho v| */
+  int outer_stop;          /* 0 = paper rule only; 1 = also |dF_g|<=rel*|F_g|, |d rho v|<=rel*|rho v|.
+                              The "paper rule" is read as  sum_g |dW_g| (c_hat/c) dt <= outer_tol * max(sum_g |R_g|, E_tot):
+                              a deviation from the literal text of PAPER.md:465 ("below 1e-13 sum R_g AND 1e-13 E_tot",
+                              i.e. the smaller of the two), which cannot be met at equilibrium where sum_g R_g -> 0
+                              (reading S10).                                                              */
   double outer_rel_tol;    /* rel of outer_stop == 1 (1e-12)                                   */
   /* ---- opacities that depend on the gas temperature: evaluated at every trial T of the Newton iteration ---- */
   int opacity_kind;        /* 0 = the table (kappa_lo, alpha) above, independent of T;
