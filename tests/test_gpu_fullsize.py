@@ -8,7 +8,7 @@ import pytest
 
 from paper_2407_18304_b200 import workloads as W
 
-from parity_util import assert_parity, oracle_model
+from parity_util import afloor_quasi_newton, assert_parity, oracle_model
 
 pytestmark = pytest.mark.gpu
 
@@ -21,21 +21,29 @@ def _sample_indices(n: int, k: int):
     return idx
 
 
-@pytest.mark.parametrize("index", [2, 3, 4, 5])
-def test_full_size_sampled_parity(oracle_lib, index):
+@pytest.mark.parametrize("index,variant", [(2, "default"), (3, "default"), (4, "default"), (5, "default"),
+                                           (4, "ktemp"), (4, "source"), (3, "free_slope"), (3, "edge_table")])
+def test_full_size_sampled_parity(oracle_lib, index, variant):
+    """`variant`: the model options of SURVEY 8(f) as bench.py --variant builds them, at the full size of the workload."""
     import torch
+
+    import bench
 
     if not torch.cuda.is_available():
         pytest.fail("GPU test selected but no CUDA device is visible")
     from paper_2407_18304_b200 import binding
 
-    wl = W.workload(index)
+    wl = bench.apply_variant(W.workload(index), variant)
     n = wl.ncells
+    quasi = variant in ("ktemp", "free_slope", "edge_table")
     free, _ = torch.cuda.mem_get_info()
     if free < 1.3 * wl.state_bytes() + (2 << 30):
         pytest.skip("not enough free device memory for the full-size state")
     dev = wl.make_state(device="cuda")
-    idx = _sample_indices(n, SAMPLES[index])
+    if variant == "source":
+        g = torch.Generator(device="cuda").manual_seed(99)
+        dev["Srad"] = dev["Erad"] * (2.0 * torch.rand(dev["Erad"].shape, generator=g, device="cuda", dtype=torch.float64))
+    idx = _sample_indices(n, SAMPLES[index] if variant == "default" else SAMPLES[index] // 2)
     tidx = torch.from_numpy(idx).cuda()
     take = lambda st: {k: (None if v is None else np.ascontiguousarray(v.index_select(v.dim() - 1, tidx).cpu().numpy()))
                        for k, v in st.items()}                                                  # noqa: E731
@@ -46,6 +54,8 @@ def test_full_size_sampled_parity(oracle_lib, index):
     E1, P1 = torch.empty_like(E0), torch.empty_like(P0)
     dt = wl.dt_of_call(0)
     ctx.conserved_totals(dev, wl.c, wl.c_hat, E0, P0)
+    if variant == "source":                        # conserved: E_gas + (c/c_hat) sum (E_g - S_g)
+        E0 += (wl.c / wl.c_hat) * dev["Srad"].sum(0)
     Es = dev["Egas"].abs() + (wl.c / wl.c_hat) * dev["Erad"].abs().sum(0)
     Ps = dev["mom"].pow(2).sum(0).sqrt() + dev["Frad"].pow(2).sum(0).sqrt().sum(0) / (wl.c * wl.c_hat)
     ctx.source_update(dev, dt, wl.c, wl.c_hat)
@@ -65,7 +75,12 @@ def test_full_size_sampled_parity(oracle_lib, index):
     got = take(dev)
     ref = {k: (None if v is None else v.copy()) for k, v in st0.items()}
     oracle_lib.source_update(oracle_model(oracle_lib, wl), ref, dt, wl.c, wl.c_hat)
-    assert_parity(ref, got, st0, wl.c, wl.c_hat, label=f"{wl.name} full size, {len(idx)} sampled cells")
+    scale = dict(st0)
+    if variant == "source":
+        scale["Erad"] = st0["Erad"] + st0["Srad"]
+    assert_parity({k: v for k, v in ref.items() if k != "Srad"}, got, scale, wl.c, wl.c_hat,
+                  label=f"{wl.name} full size, {len(idx)} sampled cells",
+                  afloor=afloor_quasi_newton(wl.newton_tol) if quasi else 1e-14)
     ctx.free()
     del dev, E0, P0, E1, P1, Es, Ps
     torch.cuda.empty_cache()
