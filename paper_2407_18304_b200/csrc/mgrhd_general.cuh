@@ -94,7 +94,7 @@ source_update_general_kernel(const __grid_constant__ Params P, const __grid_cons
   const int Nq = P.Nq;
   const long long n = P.ncells, stride = P.stride;
   const double dt = P.dt, c = P.c, chat = P.c_hat;
-  const double c_over_chat = c / chat, cdt = chat * dt, icc = 1.0 / (c * chat);
+  const double c_over_chat = c / chat, cdt = chat * dt, icc = 1.0 / (c * chat), inv_c = 1.0 / c, inv_cdt = 1.0 / cdt;
   const double NaN = __longlong_as_double(0x7ff8000000000000ll);
   const long long nwarps = ((long long)gridDim.x * blockDim.x) >> 5;
   const long long warp0 = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
@@ -122,7 +122,7 @@ source_update_general_kernel(const __grid_constant__ Params P, const __grid_cons
     const double momt0 = S.mom[0][cell], momt1 = S.mom[1][cell], momt2 = S.mom[2][cell];
     const double Egas_t = S.Egas[cell];
     const double chis = rho * ks, inv_rho = 1.0 / rho;
-    const double Cv = rho * P.cv_over_rho;
+    const double Cv = rho * P.cv_over_rho, inv_Cv = 1.0 / Cv;
     double Et[GPL], Sg[GPL], R[GPL], Ft0[GPL], Ft1[GPL], Ft2[GPL], Fk0[GPL], Fk1[GPL], Fk2[GPL];
     double Fn0[GPL], Fn1[GPL], Fn2[GPL], Enew[GPL];
     double sumEtS = 0.0;
@@ -152,15 +152,16 @@ source_update_general_kernel(const __grid_constant__ Params P, const __grid_cons
       double vF[GPL];
 #pragma unroll
       for (int k = 0; k < GPL; ++k) vF[k] = fma(v0, Fk0[k], fma(v1, Fk1[k], v2 * Fk2[k]));
-      if (!((Egs - Ekin) / Cv > 0.0)) {                                // invalid state: stop here (S9)
+      if (!((Egs - Ekin) * inv_Cv > 0.0)) {                              // invalid state: stop here (S9)
         if (lane == 0) atomicAdd(&stats[kStatTNonPos], 1ull);
         break;
       }
       // ---- inner Newton-Raphson iteration on x = (E_gas, R_1..R_Nq) (Eq. 41-50) ---------------------
       for (int it = 0;; ++it) {
-        const double T = (Egs - Ekin) / Cv;
+        const double T = (Egs - Ekin) * inv_Cv;
+        const double invT = 1.0 / T;
         const double T2 = T * T, aT4 = P.a_rad * T2 * T2;
-        const double beta = P.h_over_k / T;
+        const double beta = P.h_over_k * invT;
         // a1: edge functions at the lane's upper edges; the lower edge comes from the left, edge 0 from an
         // evaluation of its own (lane 0)
         // (through the one out-of-line copy of the three branches: this kernel is bound by instruction fetch --
@@ -222,7 +223,7 @@ source_update_general_kernel(const __grid_constant__ Params P, const __grid_cons
             alpha[k] = log(chi_hi[k] / chi_lo[k]) / lnr[k];                        // Eq. 20
           }
         } else {
-          const double f = G.opacity_kind == 1 ? pow(T * P.inv_T_ref, P.p_T) : 1.0;
+          const double f = G.opacity_kind == 1 ? exp(P.p_T * log(T * P.inv_T_ref)) : 1.0;
 #pragma unroll
           for (int k = 0; k < GPL; ++k) {
             alpha[k] = al_tab[k];
@@ -250,8 +251,14 @@ source_update_general_kernel(const __grid_constant__ Params P, const __grid_cons
             chiB[k] = chi_lo[k];                                                   // PC, Eq. 17
             chiE[k] = chi_lo[k];
           } else {
-            chiB[k] = chi_lo[k] * eq30_bracket(alpha[k] + aB[k] + 1.0, lnr[k]) / eq30_bracket(aB[k] + 1.0, lnr[k]);
-            chiE[k] = chi_lo[k] * eq30_bracket(alpha[k] + aE[k] + 1.0, lnr[k]) / eq30_bracket(aE[k] + 1.0, lnr[k]);
+            // Eq. 30; the second bracket is ln r for alpha_Q = -1, and with the fixed slope chi_E = chi_B
+            const double bB = aB[k] + 1.0;
+            chiB[k] = chi_lo[k] * eq30_bracket(alpha[k] + bB, lnr[k]) / (bB == 0.0 ? lnr[k] : eq30_bracket(bB, lnr[k]));
+            chiE[k] = chiB[k];
+            if (G.spectrum == 1) {
+              const double bE = aE[k] + 1.0;
+              chiE[k] = chi_lo[k] * eq30_bracket(alpha[k] + bE, lnr[k]) / (bE == 0.0 ? lnr[k] : eq30_bracket(bE, lnr[k]));
+            }
           }
           // a2: Doppler boundary term Delta_g(nu chi_0 B_nu) per unit a_R T^4 (Eq. 22)
           const double P3 = fma(chi_hi[k], hx[k], -chi_lo[k] * lx[k]);
@@ -265,13 +272,15 @@ source_update_general_kernel(const __grid_constant__ Params P, const __grid_cons
           if (vg[k] && evals == 0) { n_guard += guard ? 1u : 0u; n_den += denbad ? 1u : 0u; }
           chiF[k] = cf;
           // a4: work term, Eq. 42 solved for E_g, residuals of Eq. 41
-          W[k] = (1.0 + alpha[k]) * cf * vF[k] / c;
-          const double ratio = chiB[k] / chiE[k];
-          const double Eg = ratio * Bt[k] + W[k] / (c * chiE[k]) - R[k] / (cdt * chiE[k]);
+          W[k] = (1.0 + alpha[k]) * cf * vF[k] * inv_c;
+          const double inv_chiE = 1.0 / chiE[k];
+          const double ratio = chiB[k] * inv_chiE;
+          const double itau = inv_cdt * inv_chiE;                                   // 1/(c_hat dt chi_E)
+          const double Eg = fma(ratio, Bt[k], W[k] * (inv_c * inv_chiE)) - R[k] * itau;
           FR[k] = vg[k] ? Eg - Et[k] - (R[k] + Sg[k]) : 0.0;
           // a5: Jacobian, Eq. 44-47 (d(chi_B/chi_E)/dT = 0), q = -1/J_gg
-          qg[k] = 1.0 / (1.0 / (cdt * chiE[k]) + 1.0);
-          jg0[k] = ratio * (aT4 * fbd / T) / Cv;                                   // (4 Bt - Db)/T / C_v
+          qg[k] = 1.0 / (itau + 1.0);
+          jg0[k] = ratio * (aT4 * fbd * invT) * inv_Cv;                            // (4 Bt - Db)/T / C_v
           AG[k] = aT4 * fma(chiB[k], dY[k], P3 * (-1.0 / 3.0));                    // chi_B Bt - D/3 (Eq. 51 source)
           if (vg[k]) {
             sumR += R[k];
@@ -297,7 +306,8 @@ source_update_general_kernel(const __grid_constant__ Params P, const __grid_cons
         // Newton step: eliminate the gas row of the arrowhead Jacobian (Eq. 48)
         const double dx0 = (-FG - c_over_chat * SFRq) / fma(c_over_chat, SJq, 1.0);
         double lam = 1.0;
-        for (int h = 0; h < 10 && !((Egs + lam * dx0 - Ekin) / Cv > 0.0); ++h) {   // S9
+#pragma unroll 1
+        for (int h = 0; h < 10 && !((Egs + lam * dx0 - Ekin) * inv_Cv > 0.0); ++h) {   // S9
           lam *= 0.5;
           if (lane == 0) atomicAdd(&stats[kStatTNonPos], 1ull);
         }
@@ -324,9 +334,10 @@ source_update_general_kernel(const __grid_constant__ Params P, const __grid_cons
         closure_vP(P.closure, Enew[k], Fk0[k], Fk1[k], Fk2[k], v0, v1, v2, c, p0, p1, p2);
         const double w = (1.0 + alpha[k]) * chiE[k];
         const double dn = fma(cdt, chiF[k], 1.0);
-        Fn0[k] = fma(cdt, fma(v0, AG[k], w * p0), Ft0[k]) / dn;
-        Fn1[k] = fma(cdt, fma(v1, AG[k], w * p1), Ft1[k]) / dn;
-        Fn2[k] = fma(cdt, fma(v2, AG[k], w * p2), Ft2[k]) / dn;
+        const double inv_dn = 1.0 / dn;
+        Fn0[k] = fma(cdt, fma(v0, AG[k], w * p0), Ft0[k]) * inv_dn;
+        Fn1[k] = fma(cdt, fma(v1, AG[k], w * p1), Ft1[k]) * inv_dn;
+        Fn2[k] = fma(cdt, fma(v2, AG[k], w * p2), Ft2[k]) * inv_dn;
         if (vg[k]) {
           dF0 += Fn0[k] - Ft0[k]; dF1 += Fn1[k] - Ft1[k]; dF2 += Fn2[k] - Ft2[k];
           if (P.outer_stop == 1 &&
@@ -343,7 +354,7 @@ source_update_general_kernel(const __grid_constant__ Params P, const __grid_cons
 #pragma unroll
       for (int k = 0; k < GPL; ++k) {
         const double vFn = fma(vn0, Fn0[k], fma(vn1, Fn1[k], vn2 * Fn2[k]));
-        const double Wn = (1.0 + alpha[k]) * chiF[k] * vFn / c;
+        const double Wn = (1.0 + alpha[k]) * chiF[k] * vFn * inv_c;
         if (vg[k]) dW += fabs(Wn - W[k]);
       }
       dW = warp_sum(dW);
