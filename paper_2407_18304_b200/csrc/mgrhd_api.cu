@@ -5,6 +5,7 @@
 #include <cuda_runtime.h>
 
 #include <cmath>
+#include <cstdint>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
@@ -477,9 +478,15 @@ int mgrhd_source_update_host(mgrhd_ctx* ctx, const mgrhd_state* s, long long n, 
 
 static int launch_transport(mgrhd_ctx* ctx, const StatePtrs& src, const StatePtrs& dst, long long nx, double dx,
                             double wdt, double c, double chat, int bc, cudaStream_t st) {
-  const long long tiles = (nx + kTransportTile - 3) / (kTransportTile - 2);
+  // two cells per thread (16-byte accesses) when every group row starts on a 16-byte boundary
+  const bool v2 = nx % 2 == 0 && nx >= 4 && ((uintptr_t)src.Erad % 16 == 0) && ((uintptr_t)dst.Erad % 16 == 0) &&
+                  ((uintptr_t)src.Frad[0] % 16 == 0) && ((uintptr_t)src.Frad[1] % 16 == 0) && ((uintptr_t)src.Frad[2] % 16 == 0) &&
+                  ((uintptr_t)dst.Frad[0] % 16 == 0) && ((uintptr_t)dst.Frad[1] % 16 == 0) && ((uintptr_t)dst.Frad[2] % 16 == 0);
+  const long long per = (v2 ? 2 : 1) * (kTransportTile - 2);
+  const long long tiles = (nx + per - 1) / per;
   dim3 grid((unsigned)tiles, (unsigned)ctx->P.Nq);
-  transport_add_kernel<<<grid, kTransportTile, 0, st>>>(src, dst, ctx->P.closure, nx, nx, nx, wdt / dx, c, chat, bc);
+  if (v2) transport_add_kernel<2><<<grid, kTransportTile, 0, st>>>(src, dst, ctx->P.closure, nx, nx, nx, wdt / dx, c, chat, bc);
+  else transport_add_kernel<1><<<grid, kTransportTile, 0, st>>>(src, dst, ctx->P.closure, nx, nx, nx, wdt / dx, c, chat, bc);
   ctx->launches++;
   ctx->last_stream = st;
   CU(cudaGetLastError());

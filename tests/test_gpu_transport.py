@@ -34,7 +34,7 @@ def copy(st):
     return {k: (None if v is None else v.copy()) for k, v in st.items()}
 
 
-@pytest.mark.parametrize("nx", [1, 2, 3, 254, 255, 1000 + 13, 5 * 254 + 1])
+@pytest.mark.parametrize("nx", [1, 2, 3, 4, 6, 254, 255, 508, 510, 1000 + 13, 2 * 508 + 2, 5 * 254 + 1])   # odd: one cell per thread; even: two (16-byte accesses)
 @pytest.mark.parametrize("closure,bc,chat_frac", [(0, 0, 1.0), (0, 1, 0.2), (1, 0, 0.5)])
 def test_transport_add_parity(gpu, oracle_lib, nx, closure, bc, chat_frac):
     import torch
@@ -65,7 +65,7 @@ def test_transport_add_parity(gpu, oracle_lib, nx, closure, bc, chat_frac):
         assert np.abs(got["Erad"] - st0["Erad"]).max() > 0
 
 
-@pytest.mark.parametrize("index,nx,bc", [(2, 3001, 0), (3, 1203, 1), (4, 1501, 0), (5, 517, 0)])
+@pytest.mark.parametrize("index,nx,bc", [(2, 3001, 0), (2, 3000, 1), (3, 1203, 1), (4, 1501, 0), (4, 1500, 0), (5, 517, 0)])
 def test_imex_step_parity(gpu, oracle_lib, index, nx, bc):
     import torch
 
