@@ -29,10 +29,12 @@
 // source term S_g; opacities evaluated at the
 // trial temperature -- kappa_g (T/T_ref)^p and edge values
 // tabulated in T with alpha from Eq. 20; the PPL free-slope
-// spectrum fit of Appendix A.  The free-slope ITERATION is
-// "parity unpinned" beyond its fixed point (brute-force solve) and the
-// special cases listed in DESIGN.md: the paper does not say from which
-// iterate of E_g the slope alpha_E is taken (reading S20).
+// spectrum fit of Appendix A.  For the free-slope fit the
+// converged state is pinned (brute-force solve with the slopes recomputed at
+// the root); from which iterate of E_g the slope alpha_E is taken during the
+// iteration is a reading (S20) that only changes the iteration counts.  The
+// 1-D transport at the end of this file follows a spatial scheme the paper
+// does not give (reading S22): "parity unpinned" beyond the pins listed there.
 //
 // Notation (energy-density units, so 4*pi/c never appears):
 //   x      = h nu / (k_B T)
