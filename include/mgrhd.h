@@ -137,7 +137,7 @@ int mgrhd_source_update(mgrhd_ctx *ctx, const mgrhd_state *state_dev, long long 
 /* The same update for a state held in HOST memory (pinned or pageable): the cells are cut
  * into slabs that are copied to the device, updated and copied back on alternating streams,
  * so copies overlap kernels.  Synchronous: returns when the host arrays hold U^(t+1).
- * Scratch device memory (a few hundred MB) is owned by the context and reused. */
+ * Scratch device memory (three slabs of up to 512 MB, sized to the largest call so far) is owned by the context and reused. */
 int mgrhd_source_update_host(mgrhd_ctx *ctx, const mgrhd_state *state_host, long long ncells,
                              double dt, double c, double c_hat);
 

@@ -142,7 +142,8 @@ cudaError_t upload_tables_for_current_device() {
 }
 
 constexpr int kSlabs = 3;                       // host path: slabs in flight
-constexpr long long kSlabBytes = 96ll << 20;    // target bytes per slab
+constexpr long long kSlabBytes = 512ll << 20;   // largest slab (measured at 256^3 x 32, 3 slabs: 96 MB 444 ms, 256 MB 422,
+                                                // 512 MB 410, 768 MB 405, 1 GB unstable; 4 or more slabs, or smaller ones, are slower)
 
 }  // namespace
 
@@ -423,16 +424,21 @@ int mgrhd_source_update_host(mgrhd_ctx* ctx, const mgrhd_state* s, long long n, 
   if (n == 0) return MGRHD_OK;
   const int Nq = ctx->P.Nq;
   const long long per_cell = 6 + 5ll * Nq;     // rho, mom[3], Egas, kappa_scale, Erad, Frad[3], Srad
-  if (!ctx->slab[0]) {
+  {
+    // slab size: a third of the cells (so that three slabs are in flight), at most kSlabBytes; grown when a larger call comes
     long long sc = kSlabBytes / (8 * per_cell);
-    sc = (sc / 1024) * 1024;
-    if (sc < 1024) sc = 1024;
-    for (int j = 0; j < kSlabs; ++j) {
-      CU(cudaMalloc(&ctx->slab[j], (size_t)sc * per_cell * sizeof(double)));
-      CU(cudaMalloc(&ctx->slab_scratch[j], scratch_bytes(ctx)));
-      CU(cudaStreamCreateWithFlags(&ctx->slab_stream[j], cudaStreamNonBlocking));
+    const long long third = (n + kSlabs - 1) / kSlabs;
+    if (sc > third) sc = third;
+    sc = ((sc + 1023) / 1024) * 1024;
+    if (!ctx->slab[0] || sc > ctx->slab_cells) {
+      for (int j = 0; j < kSlabs; ++j) {
+        if (ctx->slab[j]) { CU(cudaStreamSynchronize(ctx->slab_stream[j])); CU(cudaFree(ctx->slab[j])); ctx->slab[j] = nullptr; }
+        CU(cudaMalloc(&ctx->slab[j], (size_t)sc * per_cell * sizeof(double)));
+        if (!ctx->slab_scratch[j]) CU(cudaMalloc(&ctx->slab_scratch[j], scratch_bytes(ctx)));
+        if (!ctx->slab_stream[j]) CU(cudaStreamCreateWithFlags(&ctx->slab_stream[j], cudaStreamNonBlocking));
+      }
+      ctx->slab_cells = sc;
     }
-    ctx->slab_cells = sc;
   }
   const long long sc = ctx->slab_cells;
   const size_t pitch_h = (size_t)n * sizeof(double), pitch_d = (size_t)sc * sizeof(double);
