@@ -130,3 +130,51 @@ def test_doppler_medium_steady_state_on_gpu(gpu, oracle_lib):
     assert abs(T[0] - Tref[0]) < 1e-13
     assert np.max(np.abs(got["Erad"] - ref["Erad"])) < 1e-12 * ref["Erad"].max()
     assert np.max(np.abs(got["Frad"][0] - ref["Frad"][0])) < 1e-10 * np.abs(ref["Frad"][0]).max()
+
+
+def test_imex_step_with_the_general_kernel_models(gpu, oracle_lib):
+    """The IMEX step dispatches its two source updates like mgrhd_source_update: free-slope spectrum (general kernel)."""
+    import torch
+
+    from parity_util import afloor_quasi_newton
+
+    wl = W.workload(2, ncells=700)
+    wl.spectrum = 1
+    st0 = W.to_numpy(wl.make_state())
+    dx, dt = 1.0, 0.5 / wl.c_hat
+    ref = copy(st0)
+    oracle_lib.imex_step_1d(oracle_model(oracle_lib, wl), ref, dx, dt, wl.c, wl.c_hat, 0)
+    ctx = gpu.Context.from_workload(wl)
+    U, Wk = to_dev(st0), to_dev(st0)
+    ctx.imex_step_1d(U, Wk, dx, dt, wl.c, wl.c_hat, 0)
+    torch.cuda.synchronize()
+    got = W.to_numpy(U)
+    ctx.free()
+    assert_parity(ref, got, st0, wl.c, wl.c_hat, label="IMEX step, free slope", afloor=afloor_quasi_newton(wl.newton_tol))
+
+
+def test_transport_argument_errors(gpu):
+    import torch
+
+    wl = W.workload(2, ncells=64)
+    a, b = wl.make_state(device="cuda"), wl.make_state(device="cuda")
+    ctx = gpu.Context.from_workload(wl)
+    with pytest.raises(gpu.MgrhdError, match="MGRHD_ERR_ARG"):
+        ctx.transport_add(a, a, 1.0, 1e-3, wl.c, wl.c_hat, 0)          # src and dst alias
+    with pytest.raises(gpu.MgrhdError, match="MGRHD_ERR_ARG"):
+        ctx.transport_add(a, b, 1.0, 1e-3, wl.c, wl.c_hat, 2)          # unknown boundary condition
+    with pytest.raises(gpu.MgrhdError, match="MGRHD_ERR_RANGE"):
+        ctx.transport_add(a, b, 0.0, 1e-3, wl.c, wl.c_hat, 0)          # dx <= 0
+    with pytest.raises(gpu.MgrhdError, match="MGRHD_ERR_RANGE"):
+        ctx.imex_step_1d(a, b, 1.0, 0.0, wl.c, wl.c_hat, 0)            # dt <= 0
+    with pytest.raises(gpu.MgrhdError, match="MGRHD_ERR_RANGE"):
+        ctx.imex_step_1d(a, b, 1.0, 1e-3, wl.c, 2 * wl.c, 0)           # c_hat > c
+    src = dict(a, Srad=torch.zeros_like(a["Erad"]))
+    with pytest.raises(gpu.MgrhdError, match="MGRHD_ERR_ARG"):
+        ctx.imex_step_1d(src, b, 1.0, 1e-3, wl.c, wl.c_hat, 0)         # a per-update source has no place in the two stages
+    torch.cuda.synchronize()
+    before = {k: v.clone() for k, v in a.items() if v is not None}
+    ctx.imex_step_1d(a, b, 1.0, 1e-3, wl.c, wl.c_hat, 0)               # and a valid call still works
+    torch.cuda.synchronize()
+    assert not torch.equal(before["Erad"], a["Erad"])
+    ctx.free()
