@@ -39,9 +39,10 @@ def parse_args():
     ap.add_argument("--sustained", type=int, default=0, metavar="CALLS",
                     help="BASELINE.json config 5 as stated: CALLS successive updates of the same buffers, dt varied "
                          "per call, device-timed per call, conservation residuals checked after every call")
-    ap.add_argument("--variant", default="default", choices=["default", "source", "ktemp", "free_slope", "edge_table"],
+    ap.add_argument("--variant", default="default", choices=["default", "source", "ktemp", "free_slope", "edge_table", "literal_units"],
                     help="model option on top of the workload (SURVEY 8(f) rows): S_g present; kappa (T/T_ref)^1.5; "
-                         "free-slope spectrum fit; edge opacities tabulated in T with alpha from Eq. 20")
+                         "free-slope spectrum fit; edge opacities tabulated in T with alpha from Eq. 20; the survey's "
+                         "variant L: literal units a_R = c = 1 (radiation inertia q >> 1) with the implicit-in-v outer stage")
     ap.add_argument("--imex", action="store_true",
                     help="SURVEY 8(f) NEXT-3: time the explicit 1-D transport kernel (HBM roofline) and whole two-stage "
                          "IMEX steps (Eq. 35-36) on the workload read as one periodic row of cells")
@@ -107,7 +108,7 @@ class ClockSampler:
 # CPU oracle legs (the only places bench.py touches oracle/)
 # --------------------------------------------------------------------------------------
 def oracle_model(oracle, wl):
-    extra = {k: getattr(wl, k) for k in ("spectrum", "opacity_kind", "T_ref", "p_T", "lnT0", "dlnT", "lnk_edge") if hasattr(wl, k)}
+    extra = {k: getattr(wl, k) for k in ("spectrum", "opacity_kind", "T_ref", "p_T", "lnT0", "dlnT", "lnk_edge", "outer_mode") if hasattr(wl, k)}
     return oracle.OracleModel(wl.edges, wl.kappa_lo, wl.alpha, a_rad=wl.a_rad, k_B=wl.k_B, h_planck=wl.h_planck,
                               mean_mass=wl.mean_mass, gamma=wl.gamma, closure=wl.closure, newton_tol=wl.newton_tol,
                               newton_maxit=wl.newton_maxit, outer_maxit=wl.outer_maxit, outer_tol=wl.outer_tol,
@@ -181,6 +182,10 @@ def apply_variant(wl, variant: str):
         wl.opacity_kind = 2
         wl.lnk_edge = np.log(k_edge)[:, None] - 0.5 * lnT[None, :]
         wl.lnT0, wl.dlnT = float(lnT[0]), float(lnT[1] - lnT[0])
+    elif variant == "literal_units":           # SURVEY 8(d) "variant L": q = (4/3) sum E_g/(rho c c_hat) up to several hundred
+        wl.a_rad, wl.c, wl.dt = 1.0, 1.0, 1.0
+        wl.c_hat = wl.c_hat / 1e3 if wl.c_hat < 1e3 else 1.0
+        wl.outer_mode = 1
     if variant != "default":
         wl.name = f"{wl.name}+{variant}"
     return wl

@@ -78,6 +78,12 @@ typedef struct {
   int NT;                  /* opacity_kind 2: number of table temperatures (>= 1)                                   */
   double lnT0, dlnT;       /*                 T_j = exp(lnT0 + j dlnT), j = 0..NT-1                                 */
   const double *lnk_edge;  /*                 [Nq+1][NT] HOST, copied: ln of the specific opacity at edge e, temperature j */
+  int outer_mode;          /* 0 = the paper's outer stage: the velocity in Eq. 51 is the lagged one, a fixed-point
+                              iteration that contracts only while the radiation inertia q = (4/3) sum_g E_g/(rho c c_hat) is
+                              small;
+                              1 = "variant L" (not in the paper): the velocity in Eq. 51 is the NEW one, so
+                              Eq. 51-52 are one 3x3 linear system for v^(t+1) per outer trip.  Same converged state; converges
+                              for q >~ 1 (radiation-dominated cells, literal units) where mode 0 diverges.  General kernel.  */
 } mgrhd_opacity_model;
 
 /* Cell state, structure of arrays, float64, cell index fastest.  In mgrhd_source_update all
@@ -115,9 +121,9 @@ typedef struct {
  *   group_edges [Nq+1] HOST: nu_{g-}, ascending, >= 0; the last may be +inf.
  *   1 <= Nq <= MGRHD_MAX_GROUPS.  The context copies everything it needs (tables go to
  *   constant memory at launch); it uses the CUDA device current at the time of the call.
- * Which kernel runs: the fixed-slope spectrum with opacity_kind 0 or 1 takes the tuned kernel (L lanes
- * per cell); the free-slope spectrum and opacity_kind 2 take the general kernel (one
- * warp per cell, lane = group), which needs the values of neighbouring groups.
+ * Which kernel runs: the fixed-slope spectrum with opacity_kind 0 or 1 and outer_mode 0 takes the tuned kernel
+ * (L lanes per cell); the free-slope spectrum, opacity_kind 2 and outer_mode 1 take the general
+ * kernel (one warp per cell, lane = group), which has a cell's groups side by side in a warp.
  * Returns MGRHD_OK and *out, or a negative error (and *out = NULL). */
 int mgrhd_init(mgrhd_ctx **out, const double *group_edges, int Nq,
                const mgrhd_units *units, const mgrhd_opacity_model *model);

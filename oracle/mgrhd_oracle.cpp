@@ -222,6 +222,12 @@ void oracle_vP(int closure, double E, const double F[3], const double v[3], doub
     vP[i] = E * (0.5 * (1.0 - chi) * v[i] + 0.5 * (3.0 * chi - 1.0) * n[i] * ndotv);
 }
 
+// The closure's pressure tensor P^{ji} itself (reading S7), for the implicit-in-v outer stage.
+void oracle_P(int closure, double E, const double F[3], double c, double P[3][3]) {
+  double e[3][3] = {{1, 0, 0}, {0, 1, 0}, {0, 0, 1}};
+  for (int j = 0; j < 3; ++j) oracle_vP(closure, E, F, e[j], c, P[j]);     // row j = e_j . P
+}
+
 // Dense solve A x = b, partial-pivot LU, A row-major n x n (destroyed), b -> x.
 // Returns 0, or -1 if a zero pivot is met.
 int oracle_lu_solve(int n, double* A, double* b) {
@@ -296,6 +302,10 @@ typedef struct {
   int NT;                   // kind 2: temperatures in the table
   double lnT0, dlnT;        //         T_j = exp(lnT0 + j dlnT)
   const double* lnk_edge;   //         [Nq+1][NT] ln of the specific opacity at edge e, temperature j
+  int outer_mode;           // 0: the paper's outer stage, velocity lagged in Eq. 51;
+                            // 1: "variant L" of SURVEY 8(f) NEXT-4: v in Eq. 51 is the NEW velocity, so Eq. 51-52 are
+                            //    one 3x3 linear system for v^(t+1) per outer trip (same fixed point; converges when the
+                            //    radiation inertia q = (4/3) sum E_g/(rho c c_hat) is not small).  Not in the paper.
 } oracle_model;
 
 enum { ORACLE_HIST = 64 };
@@ -475,6 +485,35 @@ void update_cell(const oracle_model& m, double dt, double c, double chat,
 
     // O9: flux update with the lagged velocity (Eq. 51); O10: gas momentum (Eq. 52)
     double dFsum[3] = {0.0, 0.0, 0.0};
+    if (m.outer_mode == 1) {
+      // variant L: Eq. 51 with the NEW velocity, F_g^new = a_g + B_g v^new, a_g = F_g^t/dn_g,
+      // B_g = (c_hat dt/dn_g) [ (chi_B Bt - D/3) I + (1 + alpha) chi_E P_g ], dn_g = 1 + c_hat chi_F dt; inserted in Eq. 52:
+      //   [rho I + (c c_hat)^-1 sum_g B_g] v^new = (rho v)^t - (c c_hat)^-1 sum_g (a_g - F_g^t)
+      double M[9] = {rho, 0, 0, 0, rho, 0, 0, 0, rho}, rhs[3] = {mom_t[0], mom_t[1], mom_t[2]};
+      std::vector<double> Bm((size_t)Nq * 9), av((size_t)Nq * 3);
+      for (int g = 0; g < Nq; ++g) {
+        double Fg[3] = {Fk[0][g], Fk[1][g], Fk[2][g]}, P[3][3];
+        oracle_P(m.closure, Enew[g], Fg, c, P);
+        const double dn = 1.0 + chat * chiF[g] * dt, A = chiB[g] * Bt[g] - D[g] / 3.0, w = (1.0 + alpha[g]) * chiE[g];
+        for (int i = 0; i < 3; ++i) {
+          av[(size_t)g * 3 + i] = Ft[i][g] / dn;
+          rhs[i] -= (av[(size_t)g * 3 + i] - Ft[i][g]) / (c * chat);
+          for (int j = 0; j < 3; ++j) {
+            const double b = (chat * dt / dn) * ((i == j ? A : 0.0) + w * P[j][i]);
+            Bm[(size_t)g * 9 + i * 3 + j] = b;
+            M[i * 3 + j] += b / (c * chat);
+          }
+        }
+      }
+      if (oracle_lu_solve(3, M, rhs) != 0) { st.n_lu_singular++; break; }
+      for (int g = 0; g < Nq; ++g)
+        for (int i = 0; i < 3; ++i) {
+          double f = av[(size_t)g * 3 + i];
+          for (int j = 0; j < 3; ++j) f += Bm[(size_t)g * 9 + i * 3 + j] * rhs[j];
+          Fnew[i][g] = f;
+          dFsum[i] += f - Ft[i][g];
+        }
+    } else
     for (int g = 0; g < Nq; ++g) {
       double Fg[3] = {Fk[0][g], Fk[1][g], Fk[2][g]}, vP[3];
       oracle_vP(m.closure, Enew[g], Fg, v, c, vP);
@@ -484,7 +523,7 @@ void update_cell(const oracle_model& m, double dt, double c, double chat,
         dFsum[i] += Fnew[i][g] - Ft[i][g];
       }
     }
-    for (int i = 0; i < 3; ++i) mom_new[i] = mom_t[i] - dFsum[i] / (c * chat);
+    for (int i = 0; i < 3; ++i) mom_new[i] = mom_t[i] - dFsum[i] / (c * chat);   // Eq. 52 (variant L: = rho v^new up to rounding)
     trips++;
 
     // O11: outer convergence (reading S10)

@@ -54,6 +54,7 @@ class _CModel(ctypes.Structure):
         ("lnT0", ctypes.c_double),
         ("dlnT", ctypes.c_double),
         ("lnk_edge", ctypes.POINTER(ctypes.c_double)),
+        ("outer_mode", ctypes.c_int),
     ]
 
 
@@ -204,6 +205,7 @@ class OracleModel:
     lnT0: float = 0.0
     dlnT: float = 1.0
     lnk_edge: np.ndarray | None = None   # [Nq+1, NT] for opacity_kind 2
+    outer_mode: int = 0          # 0 lagged velocity (paper); 1 implicit in v ("variant L")
     _keep: list = field(default_factory=list, repr=False)
 
     def _c(self) -> _CModel:
@@ -217,7 +219,7 @@ class OracleModel:
             k.shape[0], _p(e), self.a_rad, self.k_B, self.h_planck, self.mean_mass, self.gamma, _p(k), _p(a),
             self.closure, self.newton_tol, self.newton_maxit, self.outer_maxit, self.outer_tol,
             self.outer_stop, self.outer_rel_tol, self.spectrum, self.opacity_kind, self.T_ref, self.p_T,
-            0 if t is None else t.shape[1], self.lnT0, self.dlnT, None if t is None else _p(t),
+            0 if t is None else t.shape[1], self.lnT0, self.dlnT, None if t is None else _p(t), self.outer_mode,
         )
 
 

@@ -37,7 +37,8 @@ class OpacityModel(ctypes.Structure):
                 ("newton_tol", ctypes.c_double), ("newton_maxit", ctypes.c_int), ("outer_maxit", ctypes.c_int),
                 ("outer_tol", ctypes.c_double), ("outer_stop", ctypes.c_int), ("outer_rel_tol", ctypes.c_double),
                 ("opacity_kind", ctypes.c_int), ("T_ref", ctypes.c_double), ("p_T", ctypes.c_double),
-                ("NT", ctypes.c_int), ("lnT0", ctypes.c_double), ("dlnT", ctypes.c_double), ("lnk_edge", _dp)]
+                ("NT", ctypes.c_int), ("lnT0", ctypes.c_double), ("dlnT", ctypes.c_double), ("lnk_edge", _dp),
+                ("outer_mode", ctypes.c_int)]
 
 
 class State(ctypes.Structure):
@@ -150,7 +151,7 @@ class Context:
     def __init__(self, edges, kappa_lo, alpha, *, a_rad=1.0, k_B=1.0, h_planck=1.0, mean_mass=1.0,
                  gamma=5.0 / 3.0, closure=0, spectrum=0, newton_tol=1e-11, newton_maxit=50, outer_maxit=50,
                  outer_tol=1e-13, outer_stop=1, outer_rel_tol=1e-12, opacity_kind=0, T_ref=1.0, p_T=0.0,
-                 lnT0=0.0, dlnT=1.0, lnk_edge=None):
+                 lnT0=0.0, dlnT=1.0, lnk_edge=None, outer_mode=0):
         L = load_library()
         e = np.ascontiguousarray(edges, dtype=np.float64)
         self.Nq = int(e.shape[0]) - 1
@@ -166,7 +167,7 @@ class Context:
         m = OpacityModel(null if k is None else k.ctypes.data_as(_dp), null if a is None else a.ctypes.data_as(_dp),
                          closure, spectrum, newton_tol, newton_maxit, outer_maxit, outer_tol, outer_stop, outer_rel_tol,
                          opacity_kind, T_ref, p_T, 0 if t is None else t.shape[1], lnT0, dlnT,
-                         null if t is None else t.ctypes.data_as(_dp))
+                         null if t is None else t.ctypes.data_as(_dp), outer_mode)
         h = ctypes.c_void_p()
         _check(L.mgrhd_init(ctypes.byref(h), e.ctypes.data_as(_dp), self.Nq, ctypes.byref(u), ctypes.byref(m)),
                "mgrhd_init")
@@ -179,7 +180,7 @@ class Context:
                     mean_mass=wl.mean_mass, gamma=wl.gamma, closure=wl.closure, newton_tol=wl.newton_tol,
                     newton_maxit=wl.newton_maxit, outer_maxit=wl.outer_maxit, outer_tol=wl.outer_tol,
                     outer_stop=wl.outer_stop, outer_rel_tol=wl.outer_rel_tol)
-        for key in ("spectrum", "opacity_kind", "T_ref", "p_T", "lnT0", "dlnT", "lnk_edge"):   # optional model fields
+        for key in ("spectrum", "opacity_kind", "T_ref", "p_T", "lnT0", "dlnT", "lnk_edge", "outer_mode"):   # optional model fields
             if hasattr(wl, key):
                 args[key] = getattr(wl, key)
         args.update(kw)

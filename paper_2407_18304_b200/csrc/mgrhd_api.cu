@@ -233,7 +233,7 @@ int mgrhd_init(mgrhd_ctx** out, const double* edges, int Nq, const mgrhd_units* 
                const mgrhd_opacity_model* m) {
   if (out) *out = nullptr;
   if (!out || !edges || !u || !m) return MGRHD_ERR_ARG;
-  if (m->opacity_kind < 0 || m->opacity_kind > 2) return MGRHD_ERR_ARG;
+  if (m->opacity_kind < 0 || m->opacity_kind > 2 || m->outer_mode < 0 || m->outer_mode > 1) return MGRHD_ERR_ARG;
   const bool tab = m->opacity_kind == 2;
   if (!tab && (!m->kappa_lo || !m->alpha)) return MGRHD_ERR_ARG;
   if (tab && (!m->lnk_edge || m->NT < 1)) return MGRHD_ERR_ARG;
@@ -281,6 +281,7 @@ int mgrhd_init(mgrhd_ctx** out, const double* edges, int Nq, const mgrhd_units* 
   GenParams& G = ctx->G;
   G.spectrum = m->spectrum;
   G.opacity_kind = m->opacity_kind;
+  G.outer_mode = m->outer_mode;
   G.NT = tab ? m->NT : 0;
   G.lnT0 = tab ? m->lnT0 : 0.0;
   G.inv_dlnT = tab && m->NT > 1 ? 1.0 / m->dlnT : 0.0;
@@ -292,7 +293,7 @@ int mgrhd_init(mgrhd_ctx** out, const double* edges, int Nq, const mgrhd_units* 
     if (g + 1 < Nq && edges[g] > 0.0 && std::isfinite(edges[g + 2]))     // Eq. A1 between groups g and g + 1
       G.inv_lnnb[g] = 1.0 / std::log(std::sqrt(edges[g + 2] * edges[g + 1]) / std::sqrt(edges[g + 1] * edges[g]));
   }
-  ctx->general = (m->spectrum == 1 || tab) ? 1 : 0;
+  ctx->general = (m->spectrum == 1 || tab || m->outer_mode == 1) ? 1 : 0;
   for (int g = 0; g < Nq; ++g) {
     const double a = tab ? 0.0 : m->alpha[g], k = tab ? 1.0 : m->kappa_lo[g];
     P.alpha[g] = a;

@@ -76,6 +76,25 @@ __device__ __forceinline__ void free_slopes(const GenParams& G, int Nq, int lane
   }
 }
 
+// The closure's pressure tensor in the form P^{ji} = Pa delta_ji + Pb t_j t_i (reading S7; t = F/(cE) scaled as in
+// closure_vP, Pb = 0 on the isotropic lanes), for the implicit-in-v outer stage.
+__device__ __forceinline__ void closure_P(int closure, double E, double F0, double F1, double F2, double c,
+                                          double& Pa, double& Pb, double& t0, double& t1, double& t2) {
+  const double cE0 = c * E;
+  const double sc = cE0 < 1e-200 ? 0x1p+400 : (cE0 > 1e200 ? 0x1p-400 : 1.0);
+  const double cE = cE0 * sc;
+  const bool Fzero = fma(F0, F0, fma(F1, F1, F2 * F2)) == 0.0;
+  const double r1 = 1.0 / (cE > 0.0 ? cE : 1.0);
+  t0 = F0 * sc * r1; t1 = F1 * sc * r1; t2 = F2 * sc * r1;
+  const double f2u = fma(t0, t0, fma(t1, t1, t2 * t2));
+  const bool iso = closure == 1 || !(E > 0.0) || Fzero || !(f2u > 1e-290) || !(f2u < 1e290);
+  const double f2 = f2u > 1.0 ? 1.0 : f2u;
+  const double sq = sqrt(fma(-3.0, f2, 4.0));
+  Pa = iso ? E * (1.0 / 3.0) : E * ((sq - 1.0) * (1.0 / 3.0));
+  Pb = iso ? 0.0 : E * ((2.0 - sq) / f2u);
+  if (iso) { t0 = 0.0; t1 = 0.0; t2 = 0.0; }
+}
+
 enum GenStat : int { GS_EVALS = 0, GS_TRIPS, GS_GUARD, GS_DEN, GS_COUNT };
 
 // GPL: groups per lane (1: Nq <= 32, 2: Nq <= 64).  256 threads = 8 warps = 8 cells in flight per CTA.
@@ -328,9 +347,47 @@ source_update_general_kernel(const __grid_constant__ Params P, const __grid_cons
       // ---- a7: closure + flux update with the lagged velocity (Eq. 51); a8: gas momentum (Eq. 52) ----
       double dF0 = 0.0, dF1 = 0.0, dF2 = 0.0;
       bool rel_ok = true;
+      if (G.outer_mode == 1) {
+        // "variant L": v in Eq. 51 is the NEW velocity: F_g^new = a_g + B_g v^new with a_g = F_g^t/dn_g,
+        // B_g = (c_hat dt/dn_g)[(chi_B Bt - D/3) I + (1 + alpha) chi_E P_g], and Eq. 52 becomes the 3x3 system
+        //   [rho I + (c c_hat)^-1 sum_g B_g] v^new = (rho v)^t - (c c_hat)^-1 sum_g (a_g - F_g^t)
+        double ca[GPL], cb[GPL], tt0[GPL], tt1[GPL], tt2[GPL], idn[GPL];
+        double m00 = 0, m01 = 0, m02 = 0, m11 = 0, m12 = 0, m22 = 0, r0 = 0, r1 = 0, r2 = 0;
+#pragma unroll
+        for (int k = 0; k < GPL; ++k) {
+          double Pa, Pb;
+          closure_P(P.closure, Enew[k], Fk0[k], Fk1[k], Fk2[k], c, Pa, Pb, tt0[k], tt1[k], tt2[k]);
+          const double w = (1.0 + alpha[k]) * chiE[k];
+          idn[k] = 1.0 / fma(cdt, chiF[k], 1.0);
+          ca[k] = cdt * idn[k] * fma(w, Pa, AG[k]);       // isotropic part of B_g
+          cb[k] = cdt * idn[k] * (w * Pb);                // coefficient of t t^T
+          if (vg[k]) {
+            m00 += fma(cb[k], tt0[k] * tt0[k], ca[k]); m11 += fma(cb[k], tt1[k] * tt1[k], ca[k]); m22 += fma(cb[k], tt2[k] * tt2[k], ca[k]);
+            m01 += cb[k] * tt0[k] * tt1[k]; m02 += cb[k] * tt0[k] * tt2[k]; m12 += cb[k] * tt1[k] * tt2[k];
+            r0 += Ft0[k] * idn[k] - Ft0[k]; r1 += Ft1[k] * idn[k] - Ft1[k]; r2 += Ft2[k] * idn[k] - Ft2[k];
+          }
+        }
+        m00 = fma(icc, warp_sum(m00), rho); m11 = fma(icc, warp_sum(m11), rho); m22 = fma(icc, warp_sum(m22), rho);
+        m01 = icc * warp_sum(m01); m02 = icc * warp_sum(m02); m12 = icc * warp_sum(m12);
+        r0 = momt0 - icc * warp_sum(r0); r1 = momt1 - icc * warp_sum(r1); r2 = momt2 - icc * warp_sum(r2);
+        // symmetric 3x3 solve by cofactors
+        const double c00 = m11 * m22 - m12 * m12, c01 = m02 * m12 - m01 * m22, c02 = m01 * m12 - m02 * m11;
+        const double c11 = m00 * m22 - m02 * m02, c12 = m01 * m02 - m00 * m12, c22 = m00 * m11 - m01 * m01;
+        const double idet = 1.0 / (m00 * c00 + m01 * c01 + m02 * c02);
+        const double w0 = (c00 * r0 + c01 * r1 + c02 * r2) * idet, w1 = (c01 * r0 + c11 * r1 + c12 * r2) * idet,
+                     w2 = (c02 * r0 + c12 * r1 + c22 * r2) * idet;
+#pragma unroll
+        for (int k = 0; k < GPL; ++k) {
+          const double tv = cb[k] * fma(tt0[k], w0, fma(tt1[k], w1, tt2[k] * w2));
+          Fn0[k] = fma(Ft0[k], idn[k], fma(ca[k], w0, tv * tt0[k]));
+          Fn1[k] = fma(Ft1[k], idn[k], fma(ca[k], w1, tv * tt1[k]));
+          Fn2[k] = fma(Ft2[k], idn[k], fma(ca[k], w2, tv * tt2[k]));
+        }
+      }
 #pragma unroll
       for (int k = 0; k < GPL; ++k) {
         double p0, p1, p2;
+        if (G.outer_mode != 1) {
         closure_vP(P.closure, Enew[k], Fk0[k], Fk1[k], Fk2[k], v0, v1, v2, c, p0, p1, p2);
         const double w = (1.0 + alpha[k]) * chiE[k];
         const double dn = fma(cdt, chiF[k], 1.0);
@@ -338,6 +395,7 @@ source_update_general_kernel(const __grid_constant__ Params P, const __grid_cons
         Fn0[k] = fma(cdt, fma(v0, AG[k], w * p0), Ft0[k]) * inv_dn;
         Fn1[k] = fma(cdt, fma(v1, AG[k], w * p1), Ft1[k]) * inv_dn;
         Fn2[k] = fma(cdt, fma(v2, AG[k], w * p2), Ft2[k]) * inv_dn;
+        }
         if (vg[k]) {
           dF0 += Fn0[k] - Ft0[k]; dF1 += Fn1[k] - Ft1[k]; dF2 += Fn2[k] - Ft2[k];
           if (P.outer_stop == 1 &&

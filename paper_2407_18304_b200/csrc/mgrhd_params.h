@@ -89,6 +89,7 @@ struct StatePtrs {
 struct GenParams {
   int spectrum;             // 0 fixed slope alpha_Q = -1, 1 free slope (Appendix A)
   int opacity_kind;         // 0, 1, 2 as in mgrhd_opacity_model
+  int outer_mode;           // 0 lagged velocity in Eq. 51 (paper), 1 implicit in v ("variant L")
   int NT;
   double lnT0, inv_dlnT;
   const double* lnk_edge;   // device, [Nq+1][NT]

@@ -27,7 +27,7 @@ def oracle_model(oracle, wl, **kw):
                 closure=wl.closure, newton_tol=wl.newton_tol, newton_maxit=wl.newton_maxit,
                 outer_maxit=wl.outer_maxit, outer_tol=wl.outer_tol, outer_stop=wl.outer_stop,
                 outer_rel_tol=wl.outer_rel_tol)
-    for key in ("spectrum", "opacity_kind", "T_ref", "p_T", "lnT0", "dlnT", "lnk_edge"):   # optional model fields
+    for key in ("spectrum", "opacity_kind", "T_ref", "p_T", "lnT0", "dlnT", "lnk_edge", "outer_mode"):   # optional model fields
         if hasattr(wl, key):
             args[key] = getattr(wl, key)
     args.update(kw)

@@ -41,7 +41,7 @@ def test_struct_layouts_match_header(binding):
     """ctypes mirrors: field counts/sizes implied by the header."""
     assert ctypes.sizeof(binding.Units) == 5 * 8
     assert ctypes.sizeof(binding.State) == 11 * 8            # ... + Srad
-    assert ctypes.sizeof(binding.OpacityModel) == 120        # 2 pointers, controls, then kind / T_ref / p_T / NT / lnT0 / dlnT / table
+    assert ctypes.sizeof(binding.OpacityModel) == 128        # 2 pointers, controls, kind / T_ref / p_T / NT / lnT0 / dlnT / table, outer_mode
     assert ctypes.sizeof(binding.Stats) == (9 + 2 * 64) * 8
     src = open(HEADER).read()
     assert "#define MGRHD_MAX_GROUPS 64" in src and "#define MGRHD_HIST 64" in src
@@ -77,6 +77,8 @@ def test_init_argument_errors(binding):
         _init(binding, e, k, a, spectrum=2)
     with pytest.raises(binding.MgrhdError, match="MGRHD_ERR_ARG"):
         _init(binding, e, k, a, opacity_kind=3)
+    with pytest.raises(binding.MgrhdError, match="MGRHD_ERR_ARG"):
+        _init(binding, e, k, a, outer_mode=2)
     with pytest.raises(binding.MgrhdError, match="MGRHD_ERR_RANGE"):
         _init(binding, e, k, a, opacity_kind=1, T_ref=0.0, p_T=1.5)
     with pytest.raises(binding.MgrhdError, match="MGRHD_ERR_ARG"):

@@ -248,3 +248,27 @@ def test_eq62_table_in_cgs_units(gpu, oracle_lib, Nq):
     check(ref, got, st0, wl, gs, os_, f"Eq. 62 table, CGS, Nq={Nq}")
     rE, rP = conservation_residual(st0, got, c, c)
     assert rE <= 1e-13 and rP <= 1e-13
+
+
+# ---------------------------------------------------------------------------------------------------
+# outer_mode 1 ("variant L"): implicit-in-v outer stage (general kernel)
+# ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("index,n,literal", [(2, 1001, True), (2, 1001, False), (4, 601, False), (5, 203, False)])
+def test_variant_L_parity(gpu, oracle_lib, index, n, literal):
+    """Literal units (a_R = c = 1: radiation inertia q up to several hundred, where the lagged-velocity outer loop of
+    PAPER.md:453-467 diverges) and the scaled units of the BASELINE workloads, both groups-per-lane instantiations."""
+    wl = W.workload(index, ncells=n)
+    if literal:
+        wl.a_rad, wl.c, wl.c_hat, wl.dt = 1.0, 1.0, 1.0, 1.0
+    wl.outer_mode = 1
+    st0 = W.to_numpy(wl.make_state())
+    dt = wl.dt_of_call(0)
+    ref, got, gs, os_ = both(gpu, oracle_lib, wl, st0, dt)
+    assert os_["n_outer_unconverged"] == 0 and os_["n_newton_unconverged"] == 0
+    check(ref, got, st0, wl, gs, os_, f"variant L, config {index}, literal={literal}")
+    rE, rP = conservation_residual(st0, got, wl.c, wl.c_hat)
+    assert rE <= 1e-13 and rP <= 1e-13
+    if not literal:      # same converged state as the paper's outer stage (tuned kernel)
+        wl0 = W.workload(index, ncells=n)
+        lag, _ = run_gpu(gpu, wl0, st0, dt)
+        assert_parity(lag, got, st0, wl.c, wl.c_hat, label="variant L vs lagged")

@@ -365,3 +365,70 @@ def test_free_slope_conserves_energy_and_momentum(oracle_lib):
     rE, rP = conservation_residual(st0, st, wl.c, wl.c_hat)
     assert rE <= 1e-13 and rP <= 1e-13
     assert s["n_newton_unconverged"] == 0
+
+
+# ---------------------------------------------------------------------------
+# outer_mode 1 ("variant L"): Eq. 51-52 solved implicitly in the velocity -- same root, converges at large radiation inertia
+# ---------------------------------------------------------------------------
+def test_variant_L_converges_to_the_brute_force_root_where_the_lagged_iteration_diverges(oracle_lib):
+    """A radiation-dominated cell in literal units (a_R = c = 1): q = (4/3) sum E_g/(rho c c_hat) ~ 50, far outside
+    the premise q << 1 of the lagged-velocity outer loop, which does not converge here.  The implicit-in-v
+    outer stage reaches the root of the full system (30-digit solve, same residual function as every other case)."""
+    Nq, edges, alpha, kap = 3, [0.05, 0.6, 3.0, 20.0], [-2.0, 1.0, -3.5], [4.0, 0.3, 2.0]
+    a_rad, c, chat, dt, rho, T0 = 1.0, 1.0, 1.0, 0.7, 0.05, 1.3
+    mom0 = rho * np.array([0.02, -0.01, 0.03])
+    Egas0 = 1.5 * rho * T0 + 0.5 * (mom0 ** 2).sum() / rho
+    E0 = np.array([float(a_rad * (1.1 * T0) ** 4 * mp_dY(edges[g] / (1.1 * T0), edges[g + 1] / (1.1 * T0))) for g in range(Nq)])
+    F0 = np.array([[0.2, -0.1, 0.05], [0.1, 0.3, -0.2], [-0.05, 0.02, 0.1]]) * c * E0[:, None]
+    q = 4.0 / 3.0 * E0.sum() / (rho * c * chat)
+    assert q > 30
+    lag = one_cell_state(Nq, rho, mom0, Egas0, E0, F0.T.copy())
+    s0 = oracle_lib.source_update(oracle_lib.OracleModel(np.array(edges), np.array(kap), np.array(alpha), a_rad=a_rad), lag, dt, c, chat)
+    assert s0["n_outer_unconverged"] + s0["n_T_nonpositive_steps"] + s0["n_newton_unconverged"] > 0 or not np.isfinite(lag["Erad"]).all()
+    m = oracle_lib.OracleModel(np.array(edges), np.array(kap), np.array(alpha), a_rad=a_rad, outer_mode=1)
+    st = one_cell_state(Nq, rho, mom0, Egas0, E0, F0.T.copy())
+    s1 = oracle_lib.source_update(m, st, dt, c, chat)
+    assert s1["n_outer_unconverged"] == 0 and s1["n_newton_unconverged"] == 0 and s1["n_T_nonpositive_steps"] == 0
+    assert 2 <= s1["outer_trips_total"] <= 25
+    M = mp.mpf
+    p = dict(Nq=Nq, c=M(c), chat=M(chat), dt=M(dt), rho=M(rho), Cv=M(1.5) * M(rho), a_rad=M(a_rad), h=M(1), kB=M(1),
+             edges=[M(e) for e in edges], alpha=[M(a) for a in alpha], chi_lo=[M(rho) * M(k) for k in kap],
+             E0=[M(e) for e in E0], F0=[[M(f) for f in F0[g]] for g in range(Nq)], Egas0=M(Egas0), mom0=[M(t) for t in mom0])
+    Etot = Egas0 + E0.sum()
+    scale = [Etot] + [np.linalg.norm(mom0) + np.abs(F0).sum() / (c * chat)] * 3 + [Etot] * Nq + [c * Etot] * (3 * Nq)
+    _brute(oracle_lib, m, st, p, Nq, scale, rtol=1e-10, atol=1e-12)
+    assert abs(st["Egas"][0] - Egas0) > 1e-3 * Egas0
+
+
+@pytest.mark.parametrize("idx,n", [(2, 150), (4, 100)])
+def test_variant_L_equals_the_lagged_iteration_at_small_radiation_inertia(oracle_lib, idx, n):
+    """Both outer stages converge to the same state (the root of Eq. 37-40); on the BASELINE workloads (q <= 3e-3) they
+    agree to the parity tolerance, and the implicit one needs no more trips."""
+    wl = W.workload(idx, ncells=n)
+    st0 = W.to_numpy(wl.make_state())
+    a, b = _copy(st0), _copy(st0)
+    sa = oracle_lib.source_update(oracle_model(oracle_lib, wl), a, wl.dt, wl.c, wl.c_hat)
+    sb = oracle_lib.source_update(oracle_model(oracle_lib, wl, outer_mode=1), b, wl.dt, wl.c, wl.c_hat)
+    Etot = st0["Egas"] + st0["Erad"].sum(0)
+    assert np.max(np.abs(a["Erad"] - b["Erad"]) / Etot) < 1e-12
+    assert np.max(np.abs(a["Egas"] - b["Egas"]) / Etot) < 1e-12
+    assert np.max(np.abs(a["Frad"] - b["Frad"]) / (1e-10 * np.abs(a["Frad"]) + 1e-12 * wl.c * Etot)) < 1.0
+    assert np.max(np.abs(a["mom"] - b["mom"]) / np.abs(a["mom"]).max()) < 1e-10
+    assert sb["outer_trips_total"] <= sa["outer_trips_total"] and sb["n_outer_unconverged"] == 0
+
+
+def test_variant_L_on_literal_units_conserves_and_converges(oracle_lib):
+    """SURVEY 8(d) "variant L": config 2 with the literal units a_R = c = 1 (q up to several hundred): every cell converges
+    in a handful of trips and energy and momentum are conserved to round-off; the lagged iteration fails on most cells."""
+    wl = W.workload(2, ncells=300)
+    wl.a_rad, wl.c, wl.c_hat, wl.dt = 1.0, 1.0, 1.0, 1.0
+    st0 = W.to_numpy(wl.make_state())
+    st = _copy(st0)
+    s = oracle_lib.source_update(oracle_model(oracle_lib, wl, outer_mode=1), st, wl.dt, wl.c, wl.c_hat)
+    assert s["n_outer_unconverged"] == 0 and s["n_newton_unconverged"] == 0 and s["n_T_nonpositive_steps"] == 0
+    assert max(i for i, cnt in enumerate(s["outer_hist"]) if cnt) <= 20
+    rE, rP = conservation_residual(st0, st, wl.c, wl.c_hat)
+    assert rE <= 1e-13 and rP <= 1e-13
+    lag = _copy(st0)
+    s0 = oracle_lib.source_update(oracle_model(oracle_lib, wl), lag, wl.dt, wl.c, wl.c_hat)
+    assert s0["n_outer_unconverged"] + s0["n_T_nonpositive_steps"] > 50
