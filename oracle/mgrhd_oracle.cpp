@@ -35,6 +35,9 @@
 // iteration is a reading (S20) that only changes the iteration counts.  The
 // 1-D transport at the end of this file follows a spatial scheme the paper
 // does not give (reading S22): "parity unpinned" beyond the pins listed there.
+// outer_mode 1 ("variant L", not in the paper) solves
+// Eq. 51-52 implicitly in the velocity; its converged state is the same root
+// of Eq. 37-40 and is pinned by the same brute-force solve.
 //
 // Notation (energy-density units, so 4*pi/c never appears):
 //   x      = h nu / (k_B T)
