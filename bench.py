@@ -357,11 +357,11 @@ def run_ours(args) -> None:
     except Exception:
         pass
     hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
-    counted = flops_per_launch > 0            # the general kernel (free slope, edge table) is not instrumented
+    counted = flops_per_launch > 0
     roofline = {
         "bound": "alu", "achieved": achieved_tflops if counted else None, "peak": peak_tflops, "unit": "TFLOP/s",
         "frac": achieved_tflops / peak_tflops if counted else None,
-        "note": None if counted else "general kernel (one warp per cell): algorithmic flops not instrumented; see the HBM figures",
+        "note": None if counted else "no flop count returned by the instrumented pass",
         "traffic": traffic,
         "traffic_source": traffic_src and f"profiles/{traffic_src} (ncu --set full, scaled linearly in cells; kernel sources sha {kernel_source_sha()})",
         "peak_source": "FP64 FMA rate measured in this run by mgrhd_measure_dfma_peak (x2 flop/FMA)",

@@ -363,8 +363,13 @@ static int launch_update(mgrhd_ctx* ctx, const StatePtrs& S, long long n, long l
     long long gb = (n + 7) / 8;
     const long long cap = (long long)ctx->sm_count * 8;
     if (gb > cap) gb = cap;
-    if (P.Nq <= 32) source_update_general_kernel<1><<<(unsigned)gb, 256, 0, st>>>(P, ctx->G, S, ctx->d_stats);
-    else source_update_general_kernel<2><<<(unsigned)gb, 256, 0, st>>>(P, ctx->G, S, ctx->d_stats);
+    if (P.Nq <= 32) {
+      if (count) source_update_general_kernel<1, true><<<(unsigned)gb, 256, 0, st>>>(P, ctx->G, S, ctx->d_stats);
+      else source_update_general_kernel<1, false><<<(unsigned)gb, 256, 0, st>>>(P, ctx->G, S, ctx->d_stats);
+    } else {
+      if (count) source_update_general_kernel<2, true><<<(unsigned)gb, 256, 0, st>>>(P, ctx->G, S, ctx->d_stats);
+      else source_update_general_kernel<2, false><<<(unsigned)gb, 256, 0, st>>>(P, ctx->G, S, ctx->d_stats);
+    }
     ctx->launches++;
     ctx->last_stream = st;
     CU(cudaGetLastError());

@@ -98,7 +98,9 @@ __device__ __forceinline__ void closure_P(int closure, double E, double F0, doub
 enum GenStat : int { GS_EVALS = 0, GS_TRIPS, GS_GUARD, GS_DEN, GS_COUNT };
 
 // GPL: groups per lane (1: Nq <= 32, 2: Nq <= 64).  256 threads = 8 warps = 8 cells in flight per CTA.
-template <int GPL>
+// COUNT: the instrumented instantiation also sums the algorithmic flops of DESIGN.md section 8 (with the general
+// kernel's rows for the free-slope fit, the tabulated opacities and the implicit-in-v outer stage) into kStatFlops.
+template <int GPL, bool COUNT>
 __global__ void __launch_bounds__(256)
 source_update_general_kernel(const __grid_constant__ Params P, const __grid_constant__ GenParams G,
                              const __grid_constant__ StatePtrs S, unsigned long long* __restrict__ stats) {
@@ -134,6 +136,15 @@ source_update_general_kernel(const __grid_constant__ Params P, const __grid_cons
     al_tab[k] = P.alpha[gi[k]];
   }
 
+  // algorithmic flops of one group at one trial T beyond the edge functions, and of one cell
+  unsigned long long flops = 0;
+  const bool varmeans = G.opacity_kind == 2 || G.spectrum == 1;   // chi_B, chi_E change with the iterate
+  const int fl_group = kFlopGroupEval + (G.opacity_kind == 2 ? kFlopTabEdge + kFlopTabAlpha : 0) +
+                       (varmeans ? kFlopMeansVar : 0) + (G.spectrum == 1 ? 2 * kFlopSlopeFit : 0);
+  const int fl_eq30 = G.spectrum == 1 ? 2 * kFlopEq30Free : (G.opacity_kind == 2 ? kFlopEq30Fixed : 0);
+  const int fl_cell = kFlopCellEval + (G.opacity_kind == 1 ? kFlopPowT : 0) +
+                      (G.opacity_kind == 2 ? kFlopTabCell + kFlopTabEdge : 0);
+
   for (long long cell = warp0; cell < n; cell += nwarps) {
     // ---- a0: load (the post-explicit state U^(t)) --------------------------------------
     const double rho = S.rho[cell];
@@ -158,6 +169,7 @@ source_update_general_kernel(const __grid_constant__ Params P, const __grid_cons
       sumEtS += Et[k] + Sg[k];
     }
     const double Etot = Egas_t + (chat / c) * warp_sum(sumEtS);        // Eq. 50 as printed
+    if (COUNT && lane == 0) flops += kFlopCell + kFlopCellGroup * Nq;
     double momk0 = momt0, momk1 = momt1, momk2 = momt2, momn0 = momt0, momn1 = momt1, momn2 = momt2;
     double Egs = Egas_t, Egas_new = Egas_t;
     int evals = 0, trips = 0;
@@ -191,12 +203,14 @@ source_update_general_kernel(const __grid_constant__ Params P, const __grid_cons
         for (int k = 0; k < GPL; ++k) {
           const EdgeOut o = planck_edge_call(vg[k] ? nu_hi[k] * beta : NaN);
           hy[k] = o.yz; hx[k] = o.xi; hs[k] = o.small != 0;
+          if (COUNT && vg[k]) flops += o.flops;
         }
         double e0y, e0x;
         bool e0s;
         {
           const EdgeOut o = planck_edge_call(lane == 0 ? P.nu[0] * beta : NaN);
           e0y = o.yz; e0x = o.xi; e0s = o.small != 0;
+          if (COUNT && lane == 0) flops += o.flops;
         }
         {
           const double uy = __shfl_up_sync(FULL, hy[GPL - 1], 1), ux = __shfl_up_sync(FULL, hx[GPL - 1], 1);
@@ -290,6 +304,7 @@ source_update_general_kernel(const __grid_constant__ Params P, const __grid_cons
           if (denbad) cf = chiE[k];
           if (vg[k] && evals == 0) { n_guard += guard ? 1u : 0u; n_den += denbad ? 1u : 0u; }
           chiF[k] = cf;
+          if (COUNT && vg[k]) flops += fl_group + (alpha[k] != 0.0 ? fl_eq30 : 0);
           // a4: work term, Eq. 42 solved for E_g, residuals of Eq. 41
           W[k] = (1.0 + alpha[k]) * cf * vF[k] * inv_c;
           const double inv_chiE = 1.0 / chiE[k];
@@ -316,6 +331,7 @@ source_update_general_kernel(const __grid_constant__ Params P, const __grid_cons
         }
         const double FG = Egs - Egas_t + c_over_chat * sumR;
         evals++;
+        if (COUNT && lane == 0) flops += fl_cell;
         // Eq. 49
         if (fabs(FG) / Etot < P.newton_tol && c_over_chat * sumAbsFR / Etot < P.newton_tol) break;
         if (it >= P.newton_maxit) {
@@ -333,6 +349,7 @@ source_update_general_kernel(const __grid_constant__ Params P, const __grid_cons
         Egs += lam * dx0;
 #pragma unroll
         for (int k = 0; k < GPL; ++k) R[k] += lam * (FR[k] + jg0[k] * dx0) * qg[k];
+        if (COUNT && lane == 0) flops += kFlopStepCell + kFlopStepGroup * Nq;
       }
 
       // ---- a6: energy commit ---------------------------------------------------------
@@ -406,6 +423,8 @@ source_update_general_kernel(const __grid_constant__ Params P, const __grid_cons
       dF0 = warp_sum(dF0); dF1 = warp_sum(dF1); dF2 = warp_sum(dF2);
       momn0 = momt0 - dF0 * icc; momn1 = momt1 - dF1 * icc; momn2 = momt2 - dF2 * icc;
       trips++;
+      if (COUNT && lane == 0)
+        flops += G.outer_mode == 1 ? kFlopOuterCellL + kFlopOuterGroupL * Nq : kFlopOuterCell + kFlopOuterGroup * Nq;
       // ---- a9: outer test (reading S10) ------------------------------------------------
       const double vn0 = momn0 * inv_rho, vn1 = momn1 * inv_rho, vn2 = momn2 * inv_rho;
       double dW = 0.0;
@@ -453,6 +472,10 @@ source_update_general_kernel(const __grid_constant__ Params P, const __grid_cons
     }
   }
 
+  if (COUNT) {
+    for (int off = 16; off > 0; off >>= 1) flops += __shfl_xor_sync(FULL, flops, off);
+    if (lane == 0) atomicAdd(&stats[kStatFlops], flops);
+  }
   __syncthreads();
   if (threadIdx.x < GS_COUNT && s_cnt[threadIdx.x]) {
     const int t = threadIdx.x;

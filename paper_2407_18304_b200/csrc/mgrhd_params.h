@@ -45,6 +45,16 @@ constexpr int kFlopStepGroup = 4;     // R_g += lam da_g + (lam dx0) db_g
 constexpr int kFlopOuterCell = 50;    // v, Eq. 52, commit, E_kin, outer tests, sums over the cell's lanes
 constexpr int kFlopOuterGroup = 102;  // closure (46), Eq. 51 (23), relative-change test (14), sums (9), next v.F_g and dW (10)
 constexpr int kFlopPowT = 64;         // opacity_kind 1: (T/T_ref)^p_T = exp(p ln(.)) (log 30, exp 30), chis, 1/chis
+// the general kernel's model options (exp, log, expm1 = 30 each, like exp above)
+constexpr int kFlopTabCell = 33;      // opacity_kind 2, per cell and evaluation: ln T, table position and weight
+constexpr int kFlopTabEdge = 35;      // one edge opacity: two-point interpolation in ln T (4), exp, chi scale
+constexpr int kFlopTabAlpha = 32;     // Eq. 20: ratio, log, division by ln r
+constexpr int kFlopMeansVar = 6;      // means that change with the iterate: 3 chi_B + (1+alpha) chi_E (4), chi_B/chi_E (2)
+constexpr int kFlopEq30Fixed = 34;    // Eq. 30 with alpha_Q = -1: z = alpha ln r, expm1, /alpha, /ln r, chi_lo x
+constexpr int kFlopEq30Free = 66;     // Eq. 30 with a fitted slope: two brackets (mul, expm1, div each = 32), ratio, chi_lo x
+constexpr int kFlopSlopeFit = 36;     // Eq. A1-A2 for one of B_g, E_g: Q/width, ratio, log, x 1/ln(nubar ratio), minmod (3)
+constexpr int kFlopOuterGroupL = 126; // outer_mode 1: closure tensor (34), B_g (11), 6 matrix + 3 rhs sums (30), F_g^new (21), dF sums (6), test (14), next v.F_g and dW (10)
+constexpr int kFlopOuterCellL = 107;  // outer_mode 1: kFlopOuterCell (50) + scaling the 9 sums (15), cofactors (18), determinant and reciprocal (6), v (18)
 constexpr int kFlopCell = 16;         // load-time derivations
 constexpr int kFlopCellGroup = 7;     // sum E_g, first v.F_g, E_g commit
 
