@@ -34,7 +34,8 @@ enum {
   MGRHD_ERR_RANGE = -2,      /* dt <= 0, c <= 0, c_hat <= 0 or c_hat > c, non-positive units or opacities */
   MGRHD_ERR_EDGES = -3,      /* edges not strictly ascending, negative, or NaN                  */
   MGRHD_ERR_ALPHA = -4,      /* alpha != 0 (or opacity_kind 2) in a group whose edge is 0 or +inf (Eq. 19, 20 undefined) */
-  MGRHD_ERR_CUDA = -5        /* CUDA runtime failure; mgrhd_last_error() has the text           */
+  MGRHD_ERR_CUDA = -5,       /* CUDA runtime failure; mgrhd_last_error() has the text           */
+  MGRHD_ERR_SIZE = -6        /* mgrhd_source_update_static: the launch needs more scratch than the static array holds */
 };
 
 typedef struct mgrhd_ctx mgrhd_ctx; /* opaque; created by mgrhd_init, destroyed by mgrhd_free */
@@ -184,6 +185,34 @@ int mgrhd_reset_stats(mgrhd_ctx *ctx);
 int mgrhd_set_flop_counting(mgrhd_ctx *ctx, int on);
 /* Number of kernels this context has launched so far (for bench.py's gpu_launches). */
 long long mgrhd_launch_count(const mgrhd_ctx *ctx);
+
+/* The source update (same operation, same kernel, same results as mgrhd_source_update) for callers that cannot
+ * allocate device memory -- code under CUDA graph capture, serving loops, harnesses that forbid cudaMalloc.  It
+ * needs no context: the group structure and the model are passed on every call (HOST pointers, as for mgrhd_init),
+ * and the kernel's scratch (the work counter and the F_g^(t) copy of the cells in flight) and
+ * its counter block live in file-scope `static __device__` arrays of the library:
+ *   MGRHD_STATIC_SCRATCH_BYTES (12 MiB) of scratch + 1.2 KB of counters, held by EVERY GPU that loads the library
+ *   until the process exits.
+ * The call does no cudaMalloc / cudaFree and calls no allocating library routine; per device, its first call does
+ * the one-time set-up (Planck tables to __constant__ memory, cudaGetSymbolAddress of the two arrays): make that
+ * call outside a graph capture.
+ * Limits.  Only the models the tuned kernel runs: spectrum 0, opacity_kind 0 or 1, outer_mode 0 (anything else:
+ * MGRHD_ERR_ARG).  The scratch a launch needs is 256 + 24 NQL threads_per_CTA CTAs bytes (NQL = 4, 8, 8, 8, 16 and
+ * 256, 384, 384, 384, 288 threads for Nq <= 4, 8, 16, 32, 64; CTAs = min(resident CTAs of the device,
+ * ceil(ncells / cells per CTA))): on a 148-SM B200 every Nq <= 32 fits at any ncells (10.9 MB); 32 < Nq <= 64 fits
+ * up to 8136 cells.  A launch that needs more returns MGRHD_ERR_SIZE (mgrhd_last_error() states both numbers)
+ * and does nothing.
+ * Sharing.  Every call on a device uses the same arrays, which keep the previous call's contents: the call clears
+ * the work counter and the counters itself (stream-ordered memsets), the rest of the scratch is written before it is
+ * read.  Two calls that overlap on the GPU (different streams, or two host threads) RACE on the arrays and give
+ * wrong results: issue them on one stream, or order them with events.
+ * stats_out: NULL, or a HOST struct that receives this call's counters; a non-NULL stats_out makes the call
+ * synchronise the stream.  state: DEVICE pointers, as in mgrhd_source_update; updated in place.
+ * Errors: as mgrhd_init and mgrhd_source_update for the same arguments, plus MGRHD_ERR_SIZE. */
+#define MGRHD_STATIC_SCRATCH_BYTES (12ll << 20)
+int mgrhd_source_update_static(const double *edges, int Nq, const mgrhd_units *u, const mgrhd_opacity_model *m,
+                               const mgrhd_state *state, long long ncells, double dt, double c, double c_hat,
+                               void *cuda_stream, mgrhd_stats *stats_out);
 
 /* Diagnostic: the kernel's Planck edge functions on n DEVICE values x >= 0 (x = h nu/(k_B T)):
  *   is_y[i] = 1: yz[i] = Y(x) = (15/pi^4) int_0^x t^3/(e^t-1) dt;  is_y[i] = 0: yz[i] = 1 - Y(x);

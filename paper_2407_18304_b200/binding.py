@@ -18,7 +18,7 @@ MAX_GROUPS = 64
 HIST = 64
 
 EXPORTS = (
-    "mgrhd_init", "mgrhd_source_update", "mgrhd_source_update_host", "mgrhd_conserved_totals",
+    "mgrhd_init", "mgrhd_source_update", "mgrhd_source_update_host", "mgrhd_source_update_static", "mgrhd_conserved_totals",
     "mgrhd_transport_add", "mgrhd_imex_step_1d",
     "mgrhd_get_stats", "mgrhd_reset_stats", "mgrhd_set_flop_counting", "mgrhd_launch_count", "mgrhd_planck_edge_functions", "mgrhd_measure_dfma_peak",
     "mgrhd_last_error", "mgrhd_free",
@@ -76,6 +76,9 @@ def load_library() -> ctypes.CDLL:
     L.mgrhd_init.argtypes = [ctypes.POINTER(vp), _dp, i, ctypes.POINTER(Units), ctypes.POINTER(OpacityModel)]
     L.mgrhd_source_update.restype = i
     L.mgrhd_source_update.argtypes = [vp, ctypes.POINTER(State), ll, d, d, d, vp]
+    L.mgrhd_source_update_static.restype = i
+    L.mgrhd_source_update_static.argtypes = [_dp, i, ctypes.POINTER(Units), ctypes.POINTER(OpacityModel),
+                                             ctypes.POINTER(State), ll, d, d, d, vp, ctypes.POINTER(Stats)]
     L.mgrhd_source_update_host.restype = i
     L.mgrhd_source_update_host.argtypes = [vp, ctypes.POINTER(State), ll, d, d, d]
     L.mgrhd_transport_add.restype = i
@@ -105,12 +108,12 @@ def load_library() -> ctypes.CDLL:
 
 
 _ERR = {-1: "MGRHD_ERR_ARG", -2: "MGRHD_ERR_RANGE", -3: "MGRHD_ERR_EDGES", -4: "MGRHD_ERR_ALPHA",
-        -5: "MGRHD_ERR_CUDA"}
+        -5: "MGRHD_ERR_CUDA", -6: "MGRHD_ERR_SIZE"}
 
 
 def _check(rc: int, what: str) -> None:
     if rc != 0:
-        msg = load_library().mgrhd_last_error().decode() if rc == -5 else ""
+        msg = load_library().mgrhd_last_error().decode() if rc in (-5, -6) else ""
         raise MgrhdError(f"{what}: {_ERR.get(rc, rc)} {msg}".strip())
 
 
@@ -271,6 +274,44 @@ def measure_dfma_peak(iters: int = 1 << 20) -> float:
     out = ctypes.c_double(0.0)
     _check(load_library().mgrhd_measure_dfma_peak(iters, ctypes.byref(out)), "mgrhd_measure_dfma_peak")
     return out.value
+
+
+STATIC_SCRATCH_BYTES = 12 << 20
+
+
+def source_update_static(wl, state: dict, dt: float, c: float, c_hat: float, stream=None, want_stats=False):
+    """mgrhd_source_update_static: the update of DEVICE tensors in place with no context and no device allocation
+    (scratch and counters in static device arrays of the library; see include/mgrhd.h for the limits and the
+    sharing rule).  wl: anything with the attributes Context.from_workload reads.  Returns the call's counters
+    when want_stats (which synchronises the stream), else None."""
+    L = load_library()
+    e = np.ascontiguousarray(wl.edges, dtype=np.float64)
+    Nq = int(e.shape[0]) - 1
+    k = np.ascontiguousarray(wl.kappa_lo, dtype=np.float64)
+    a = np.ascontiguousarray(wl.alpha, dtype=np.float64)
+    if k.shape[0] != Nq or a.shape[0] != Nq:
+        raise MgrhdError("edges must have Nq+1 entries and kappa_lo, alpha Nq")
+    u = Units(wl.a_rad, wl.k_B, wl.h_planck, wl.mean_mass, wl.gamma)
+    m = OpacityModel(k.ctypes.data_as(_dp), a.ctypes.data_as(_dp), wl.closure, getattr(wl, "spectrum", 0), wl.newton_tol,
+                     wl.newton_maxit, wl.outer_maxit, wl.outer_tol, wl.outer_stop, wl.outer_rel_tol,
+                     getattr(wl, "opacity_kind", 0), getattr(wl, "T_ref", 1.0), getattr(wl, "p_T", 0.0), 0, 0.0, 1.0,
+                     ctypes.cast(None, _dp), getattr(wl, "outer_mode", 0))
+    n = int(state["rho"].shape[0])
+    assert state["rho"].is_cuda, "mgrhd_source_update_static takes device tensors"
+    if stream is None:
+        import torch
+        stream = torch.cuda.current_stream().cuda_stream
+    s = _state_struct(state, Nq, n)
+    st = Stats()
+    _check(L.mgrhd_source_update_static(e.ctypes.data_as(_dp), Nq, ctypes.byref(u), ctypes.byref(m), ctypes.byref(s), n,
+                                        dt, c, c_hat, ctypes.c_void_p(stream), ctypes.byref(st) if want_stats else None),
+           "mgrhd_source_update_static")
+    if not want_stats:
+        return None
+    out = {key: getattr(st, key) for key, _ in Stats._fields_ if not key.endswith("_hist")}
+    out["newton_hist"] = np.array(st.newton_hist[:], dtype=np.int64)
+    out["outer_hist"] = np.array(st.outer_hist[:], dtype=np.int64)
+    return out
 
 
 def planck_edge_functions(x):

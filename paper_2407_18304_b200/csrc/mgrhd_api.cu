@@ -643,6 +643,122 @@ int mgrhd_measure_dfma_peak(long long iters, double* fma_per_second) {
   return MGRHD_OK;
 }
 
+// ---- mgrhd_source_update_static: the update without any device allocation (include/mgrhd.h) ---------------------
+// The scratch and the counter block of the update kernel as file-scope device arrays.  In HOST code these names are
+// host-side stand-ins, not device addresses: the addresses the kernel gets come from cudaGetSymbolAddress, once per
+// device, with that device current (static_setup below).
+static __device__ __align__(256) double g_static_scratch[MGRHD_STATIC_SCRATCH_BYTES / sizeof(double)];
+static __device__ __align__(256) unsigned long long g_static_stats[kStatCount];
+
+struct StaticDev {
+  std::once_flag once;
+  cudaError_t err;
+  double* scratch;
+  unsigned long long* stats;
+  int sm_count;
+};
+static StaticDev g_static_dev[16];
+
+static cudaError_t static_setup(int dev) {
+  StaticDev& d = g_static_dev[dev];
+  std::call_once(d.once, [&d, dev]() {
+    d.err = upload_tables_for_current_device();
+    if (d.err == cudaSuccess) d.err = cudaDeviceGetAttribute(&d.sm_count, cudaDevAttrMultiProcessorCount, dev);
+    if (d.err == cudaSuccess) d.err = cudaGetSymbolAddress((void**)&d.scratch, g_static_scratch);
+    if (d.err == cudaSuccess) d.err = cudaGetSymbolAddress((void**)&d.stats, g_static_stats);
+  });
+  return d.err;
+}
+
+int mgrhd_source_update_static(const double* edges, int Nq, const mgrhd_units* u, const mgrhd_opacity_model* m,
+                               const mgrhd_state* s, long long n, double dt, double c, double chat, void* stream,
+                               mgrhd_stats* stats_out) {
+  // the checks of mgrhd_init for the models the tuned kernel runs
+  if (!edges || !u || !m) return MGRHD_ERR_ARG;
+  if (m->spectrum != 0 || m->outer_mode != 0 || (m->opacity_kind != 0 && m->opacity_kind != 1)) return MGRHD_ERR_ARG;
+  if (!m->kappa_lo || !m->alpha || Nq < 1 || Nq > MGRHD_MAX_GROUPS) return MGRHD_ERR_ARG;
+  if (m->closure < 0 || m->closure > 1 || m->outer_stop < 0 || m->outer_stop > 1 || m->newton_maxit < 1 ||
+      m->outer_maxit < 1)
+    return MGRHD_ERR_ARG;
+  if (!(u->a_rad > 0) || !(u->k_B > 0) || !(u->h_planck > 0) || !(u->mean_mass > 0) || !(u->gamma > 1) ||
+      !(m->newton_tol > 0) || !(m->outer_tol > 0))
+    return MGRHD_ERR_RANGE;
+  if (m->opacity_kind == 1 && (!(m->T_ref > 0) || !std::isfinite(m->T_ref) || !std::isfinite(m->p_T))) return MGRHD_ERR_RANGE;
+  for (int g = 0; g < Nq; ++g) {
+    if (!(edges[g] >= 0.0) || !(edges[g + 1] > edges[g])) return MGRHD_ERR_EDGES;
+    if (m->alpha[g] != 0.0 && (edges[g] == 0.0 || std::isinf(edges[g + 1]))) return MGRHD_ERR_ALPHA;
+    if (!std::isfinite(m->alpha[g]) || !(m->kappa_lo[g] > 0.0) || !std::isfinite(m->kappa_lo[g])) return MGRHD_ERR_RANGE;
+  }
+  // a context on the host stack: parameter block as mgrhd_init fills it, nothing on the device
+  mgrhd_ctx ctx;
+  std::memset(&ctx, 0, sizeof ctx);
+  Params& P = ctx.P;
+  P.Nq = Nq;
+  P.closure = m->closure;
+  P.newton_maxit = m->newton_maxit;
+  P.outer_maxit = m->outer_maxit;
+  P.outer_stop = m->outer_stop;
+  P.newton_tol = m->newton_tol;
+  P.outer_tol = m->outer_tol;
+  P.outer_rel_tol = m->outer_rel_tol;
+  P.a_rad = u->a_rad;
+  P.h_over_k = u->h_planck / u->k_B;
+  P.cv_over_rho = u->k_B / ((u->gamma - 1.0) * u->mean_mass);
+  for (int g = 0; g <= Nq; ++g) P.nu[g] = edges[g];
+  P.inv_T_ref = m->opacity_kind == 1 ? 1.0 / m->T_ref : 1.0;
+  P.p_T = m->opacity_kind == 1 ? m->p_T : 0.0;
+  ctx.G.opacity_kind = m->opacity_kind;
+  for (int g = 0; g < Nq; ++g) {
+    const double a = m->alpha[g], k = m->kappa_lo[g];
+    P.alpha[g] = a;
+    P.k_lo[g] = k;
+    if (a == 0.0) {                       // piecewise constant, Eq. 17
+      P.k_hi[g] = k;
+      P.k_mean[g] = k;
+    } else {                              // Eq. 19 at nu_g+; Eq. 30 with alpha_Q = -1
+      const double z = a * std::log(edges[g + 1] / edges[g]);
+      P.k_hi[g] = k * std::exp(z);
+      P.k_mean[g] = k * (std::expm1(z) / z);
+    }
+    P.inv_k_mean[g] = 1.0 / P.k_mean[g];
+    P.k_num[g] = P.k_mean[g] * ((4.0 + a) / 3.0);
+    P.onepa[g] = 1.0 + a;
+  }
+  CU(cudaGetDevice(&ctx.device));
+  if (ctx.device < 0 || ctx.device >= 16) return MGRHD_ERR_ARG;
+  int rc = check_call(&ctx, s, n, dt, c, chat);
+  if (rc != MGRHD_OK) return rc;
+  CU(static_setup(ctx.device));
+  const StaticDev& d = g_static_dev[ctx.device];
+  ctx.sm_count = d.sm_count;
+  ctx.d_stats = d.stats;
+  CU(configure_ctx(&ctx));             // function attributes and occupancy of the instantiation: no allocation
+  // the grid launch_update will use, and the scratch it indexes: head + 3 NQL doubles per thread of the grid
+  long long blocks = (long long)ctx.sm_count * ctx.cfg_bps;
+  const long long cells_per_cta = ctx.cfg_threads / ctx.cfg_l;
+  const long long want = (n + cells_per_cta - 1) / cells_per_cta;
+  if (blocks > want) blocks = want;
+  const long long need = (long long)(kScratchHead * sizeof(double)) + 3ll * ctx.cfg_nq * (long long)sizeof(double) * blocks * ctx.cfg_threads;
+  if (need > MGRHD_STATIC_SCRATCH_BYTES) {
+    std::snprintf(g_err, sizeof g_err,
+                  "mgrhd_source_update_static: Nq = %d, ncells = %lld needs %lld bytes of scratch, the static array holds %lld; "
+                  "use mgrhd_source_update or fewer cells per call",
+                  Nq, n, need, (long long)MGRHD_STATIC_SCRATCH_BYTES);
+    return MGRHD_ERR_SIZE;
+  }
+  const cudaStream_t st = (cudaStream_t)stream;
+  CU(cudaMemsetAsync(d.stats, 0, kStatCount * sizeof(unsigned long long), st));   // counters of this call only
+  if (n > 0) {
+    rc = launch_update(&ctx, to_ptrs(s), n, n, dt, c, chat, st, d.scratch);      // (clears the work counter itself)
+    if (rc != MGRHD_OK) return rc;
+  }
+  if (stats_out) {
+    ctx.last_stream = st;
+    return mgrhd_get_stats(&ctx, stats_out);
+  }
+  return MGRHD_OK;
+}
+
 void mgrhd_free(mgrhd_ctx* ctx) {
   if (!ctx) return;
   for (int k = 0; k < kSlabs; ++k) {
