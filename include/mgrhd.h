@@ -214,11 +214,15 @@ int mgrhd_source_update_static(const double *edges, int Nq, const mgrhd_units *u
                                const mgrhd_state *state, long long ncells, double dt, double c, double c_hat,
                                void *cuda_stream, mgrhd_stats *stats_out);
 
-/* Diagnostic: the kernel's Planck edge functions on n DEVICE values x >= 0 (x = h nu/(k_B T)):
+/* Diagnostic: the kernels' Planck edge functions on n DEVICE values x >= 0 (x = h nu/(k_B T)):
  *   is_y[i] = 1: yz[i] = Y(x) = (15/pi^4) int_0^x t^3/(e^t-1) dt;  is_y[i] = 0: yz[i] = 1 - Y(x);
- *   xi[i] = (15/pi^4) x^4/(e^x-1).  (Eq. 11 applied to B_nu.)  Stream-ordered. */
+ *   xi[i] = (15/pi^4) x^4/(e^x-1).  (Eq. 11 applied to B_nu.)
+ * form 0: the per-interval polynomial rows (Y below x = 1) the update uses for Nq <= 32 and in the general kernel
+ * (free-slope spectrum, opacity_kind 2, outer_mode 1); form 1: the three-branch evaluation (Y below x = 1.25) it
+ * uses for 32 < Nq <= 64.  Other values: MGRHD_ERR_ARG.
+ * Stream-ordered. */
 int mgrhd_planck_edge_functions(const double *x_dev, long long n, double *yz_dev, double *xi_dev,
-                                int *is_y_dev, void *cuda_stream);
+                                int *is_y_dev, int form, void *cuda_stream);
 
 /* Sustained FP64 FMA rate of the current device in FMA/s (a dependent-chain-free DFMA
  * microbenchmark, `iters` FMAs per thread; used as the ALU roofline denominator). */

@@ -96,7 +96,7 @@ def load_library() -> ctypes.CDLL:
     L.mgrhd_launch_count.restype = ll
     L.mgrhd_launch_count.argtypes = [vp]
     L.mgrhd_planck_edge_functions.restype = i
-    L.mgrhd_planck_edge_functions.argtypes = [vp, ll, vp, vp, vp, vp]
+    L.mgrhd_planck_edge_functions.argtypes = [vp, ll, vp, vp, vp, i, vp]
     L.mgrhd_measure_dfma_peak.restype = i
     L.mgrhd_measure_dfma_peak.argtypes = [ll, _dp]
     L.mgrhd_last_error.restype = ctypes.c_char_p
@@ -314,14 +314,15 @@ def source_update_static(wl, state: dict, dt: float, c: float, c_hat: float, str
     return out
 
 
-def planck_edge_functions(x):
-    """mgrhd_planck_edge_functions on a CUDA float64 tensor x; returns (yz, xi, is_y) tensors."""
+def planck_edge_functions(x, form=0):
+    """mgrhd_planck_edge_functions on a CUDA float64 tensor x; returns (yz, xi, is_y) tensors.  form 0: per-interval
+    rows (Nq <= 32), 1: three branches (Nq <= 64, general kernel)."""
     import torch
 
     assert x.is_cuda and x.dtype == torch.float64 and x.is_contiguous()
     yz, xi = torch.empty_like(x), torch.empty_like(x)
     is_y = torch.empty(x.shape, dtype=torch.int32, device=x.device)
     _check(load_library().mgrhd_planck_edge_functions(x.data_ptr(), x.numel(), yz.data_ptr(), xi.data_ptr(),
-                                                      is_y.data_ptr(), ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)),
+                                                      is_y.data_ptr(), form, ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)),
            "mgrhd_planck_edge_functions")
     return yz, xi, is_y

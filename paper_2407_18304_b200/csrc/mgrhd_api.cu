@@ -114,6 +114,49 @@ void fill_planck_tables(PlanckTables& t) {
   }
 }
 
+// Reference functions of the per-interval rows, long double.
+//   x < 1:  Y/(x^3) = C (1/3 - x/8 + sum b_2n x^2n/(2n+3)),  Xi/x^3 = C x/(e^x - 1)
+//   x >= 8: Z e^x, Xi e^x = C x^4/(1 - e^-x)
+long double Yx3_host(long double x) {
+  long double s = 1.0L / 3.0L - x / 8.0L, p = 1.0L;
+  for (int n = 1; n <= 30; ++n) {
+    p *= x * x;
+    s += bern_over_fact(n) * p / (2.0L * n + 3.0L);
+  }
+  return kC15Pi4L * s;
+}
+long double Xix3_host(long double x) { return x == 0.0L ? kC15Pi4L : kC15Pi4L * x / expm1l(x); }
+long double Zex_host(long double x) { return Z_host(x) * expl(x); }
+long double Xiex_host(long double x) { return kC15Pi4L * x * x * x * x / (-expm1l(-x)); }
+
+// rows[kRows * kRowStride], layout in mgrhd_params.h
+void fill_planck_rows(double* rows) {
+  for (int j = 0; j < kRows; ++j) {
+    double* r = rows + j * kRowStride;
+    long double a, b;
+    if (j == 0) { a = 0.0L; b = 0.5L; }
+    else {
+      const int bin = (j - 1) / 8, m = (j - 1) % 8;
+      const long double lo = ldexpl(0.5L, bin), w = lo / 8.0L;
+      a = lo + m * w; b = a + w;
+    }
+    double cy[kRowTerms], cx[kRowTerms];
+    if (j == kRows - 1) {                       // x >= 64: e^-x < 2e-28, Z e^x and Xi e^x are polynomials in x
+      for (int k = 0; k < kRowTerms; ++k) { cy[k] = 0.0; cx[k] = 0.0; }
+      cy[0] = (double)(6.0L * kC15Pi4L); cy[1] = cy[0]; cy[2] = (double)(3.0L * kC15Pi4L); cy[3] = (double)kC15Pi4L;
+      cx[4] = (double)kC15Pi4L;
+      r[0] = 0.0; r[1] = 1.0;
+    } else {
+      long double (*fy)(long double) = b <= 1.0L ? Yx3_host : (b <= 8.0L ? Z_host : Zex_host);
+      long double (*fx)(long double) = b <= 1.0L ? Xix3_host : (b <= 8.0L ? Xi_host : Xiex_host);
+      cheb_fit_monomial(fy, a, b, 32, kRowTerms, cy);
+      cheb_fit_monomial(fx, a, b, 32, kRowTerms, cx);
+      r[0] = (double)(0.5L * (a + b)); r[1] = (double)(2.0L / (b - a));
+    }
+    for (int k = 0; k < kRowTerms; ++k) { r[2 + 2 * k] = cy[k]; r[3 + 2 * k] = cx[k]; }
+  }
+}
+
 std::once_flag g_tables_once[16];  // per device
 cudaError_t g_tables_err[16];
 
@@ -128,6 +171,12 @@ const PlanckTables* host_planck_tables() {
   });
   return t;
 }
+const double* host_planck_rows() {
+  static double rows[kRows * kRowStride];
+  static std::once_flag once;
+  std::call_once(once, []() { fill_planck_rows(rows); });
+  return rows;
+}
 
 cudaError_t upload_tables_for_current_device() {
   int dev = 0;
@@ -135,8 +184,11 @@ cudaError_t upload_tables_for_current_device() {
   if (e != cudaSuccess) return e;
   if (dev < 0 || dev >= 16) return cudaErrorInvalidDevice;
   const PlanckTables* t = host_planck_tables();
-  std::call_once(g_tables_once[dev], [dev, t]() {
+  const double* rows = host_planck_rows();
+  std::call_once(g_tables_once[dev], [dev, t, rows]() {
     g_tables_err[dev] = cudaMemcpyToSymbol(mgrhd_c_planck, t, 2 * sizeof(PlanckTables));
+    if (g_tables_err[dev] == cudaSuccess)
+      g_tables_err[dev] = cudaMemcpyToSymbol(mgrhd_g_rows, rows, kRows * kRowStride * sizeof(double));
   });
   return g_tables_err[dev];
 }
@@ -601,13 +653,13 @@ int mgrhd_set_flop_counting(mgrhd_ctx* ctx, int on) {
 long long mgrhd_launch_count(const mgrhd_ctx* ctx) { return ctx ? ctx->launches : 0; }
 
 int mgrhd_planck_edge_functions(const double* x_dev, long long n, double* yz_dev, double* xi_dev,
-                                int* is_y_dev, void* stream) {
-  if (n < 0 || (n > 0 && (!x_dev || !yz_dev || !xi_dev || !is_y_dev))) return MGRHD_ERR_ARG;
+                                int* is_y_dev, int form, void* stream) {
+  if (n < 0 || (n > 0 && (!x_dev || !yz_dev || !xi_dev || !is_y_dev)) || (form != 0 && form != 1)) return MGRHD_ERR_ARG;
   if (n == 0) return MGRHD_OK;
   CU(upload_tables_for_current_device());
   long long blocks = (n + 255) / 256;
   if (blocks > 4096) blocks = 4096;
-  planck_edge_kernel<<<(unsigned)blocks, 256, 0, (cudaStream_t)stream>>>(x_dev, n, yz_dev, xi_dev, is_y_dev, 0);
+  planck_edge_kernel<<<(unsigned)blocks, 256, 0, (cudaStream_t)stream>>>(x_dev, n, yz_dev, xi_dev, is_y_dev, form, 0);
   CU(cudaGetLastError());
   return MGRHD_OK;
 }

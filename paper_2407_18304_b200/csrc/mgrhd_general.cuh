@@ -11,11 +11,12 @@
 // With lane = group a neighbour is one shuffle away and the sums of Eq. 48-52 are full-warp butterflies.
 // It also runs every other option (opacity_kind 0/1, S_g), which the tests use to cross-check the two
 // kernels.  The iteration (iterates, stopping tests, guards, readings S8-S10, S19-S21 of DESIGN.md) is the
-// same as the tuned kernel's; the Planck edge functions and the closure are the same device functions.
+// same as the tuned kernel's; the Planck edge functions (row form) and the closure are the same device functions.
 //
-// Cost: every lane of a warp evaluates a different edge, so all three branches of the edge functions run
-// in every evaluation, and a cell's 4 Nq + 5 loads touch 4 Nq + 5 different sectors (cell index is the
-// fastest in the state): a feature path, measured separately, not the benchmark path.
+// Cost: every lane of a warp evaluates a different edge (hence the per-interval rows of planck_edge_t: a
+// three-branch evaluation would run every branch in every evaluation), and a cell's 4 Nq + 5 loads touch
+// 4 Nq + 5 different sectors (cell index is the fastest in the state): a feature path, measured separately
+// (DESIGN.md section 12), not the benchmark path.
 //
 // Product code; shares nothing with oracle/.
 #pragma once
@@ -33,6 +34,15 @@ __device__ __forceinline__ double warp_sum(double v) {
 __device__ __noinline__ double eq30_bracket(double q, double lnr) {
   const double z = q * lnr;
   return z == 0.0 ? lnr : expm1(z) / q;
+}
+
+// One out-of-line copy of the row evaluation (two call sites per evaluation).
+__device__ __noinline__ EdgeOut planck_edge_t_call(double x, const double* rows) {
+  EdgeOut o;
+  bool sm;
+  planck_edge_t(x, rows, o.yz, o.xi, sm, o.flops);
+  o.small = sm;
+  return o;
 }
 
 // minmod of Eq. A2.
@@ -106,6 +116,8 @@ source_update_general_kernel(const __grid_constant__ Params P, const __grid_cons
                              const __grid_constant__ StatePtrs S, unsigned long long* __restrict__ stats) {
   __shared__ unsigned int s_hist[2 * MGRHD_HIST];
   __shared__ unsigned int s_cnt[GS_COUNT];
+  __shared__ __align__(16) double s_rows[kRows * kRowStride];     // per-interval rows of the edge functions
+  for (int t = threadIdx.x; t < kRows * kRowStride; t += blockDim.x) s_rows[t] = mgrhd_g_rows[t];
   for (int t = threadIdx.x; t < 2 * MGRHD_HIST; t += blockDim.x) s_hist[t] = 0u;
   if (threadIdx.x < GS_COUNT) s_cnt[threadIdx.x] = 0u;
   __syncthreads();
@@ -194,21 +206,20 @@ source_update_general_kernel(const __grid_constant__ Params P, const __grid_cons
         const double T2 = T * T, aT4 = P.a_rad * T2 * T2;
         const double beta = P.h_over_k * invT;
         // a1: edge functions at the lane's upper edges; the lower edge comes from the left, edge 0 from an
-        // evaluation of its own (lane 0)
-        // (through the one out-of-line copy of the three branches: this kernel is bound by instruction fetch --
-        // its loop body exceeds the 32 KB the SM's instruction cache holds -- so code size comes first)
+        // evaluation of its own (lane 0).  The 32 lanes hold 32 different x, so the per-interval rows
+        // (planck_edge_t: one row per lane, no branch but e^-x) replace three warp-wide branches per evaluation.
         double hy[GPL], hx[GPL], ly[GPL], lx[GPL];
         bool hs[GPL], ls[GPL];
 #pragma unroll 1
         for (int k = 0; k < GPL; ++k) {
-          const EdgeOut o = planck_edge_call(vg[k] ? nu_hi[k] * beta : NaN);
+          const EdgeOut o = planck_edge_t_call(vg[k] ? nu_hi[k] * beta : NaN, s_rows);
           hy[k] = o.yz; hx[k] = o.xi; hs[k] = o.small != 0;
           if (COUNT && vg[k]) flops += o.flops;
         }
         double e0y, e0x;
         bool e0s;
         {
-          const EdgeOut o = planck_edge_call(lane == 0 ? P.nu[0] * beta : NaN);
+          const EdgeOut o = planck_edge_t_call(lane == 0 ? P.nu[0] * beta : NaN, s_rows);
           e0y = o.yz; e0x = o.xi; e0s = o.small != 0;
           if (COUNT && lane == 0) flops += o.flops;
         }

@@ -163,6 +163,12 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
   // the small indexed-constant cache next to the Planck coefficients (24 % misses measured).
   constexpr int TS = 10;   // row stride in doubles: 80 B puts the L rows of a step on distinct banks
   __shared__ __align__(16) double s_tab[(kMaxG + 1) * TS];
+  // Per-interval rows of the edge functions (planck_edge_t) where the instantiation leaves room for them beside its
+  // group state; the Nq <= 64 instantiation fills shared memory and keeps the three-branch planck_edge_w.
+  constexpr bool TAB = (size_t)SL_COUNT * NQL * THREADS * sizeof(double) + 6144 + kRows * kRowStride * sizeof(double) <= 227 * 1024;
+  __shared__ __align__(16) double s_rows[TAB ? kRows * kRowStride : 2];
+  if constexpr (TAB)
+    for (int t = threadIdx.x; t < kRows * kRowStride; t += THREADS) s_rows[t] = mgrhd_g_rows[t];
   for (int t = threadIdx.x; t < 2 * MGRHD_HIST; t += THREADS) s_hist[t] = 0u;
   for (int r = threadIdx.x; r <= P.Nq; r += THREADS) {
     const int g = r > 0 ? r - 1 : 0;
@@ -338,7 +344,9 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
       {
         bool sm0;
         int f0;
-        planck_edge0(ev ? P.nu[0] * beta : __longlong_as_double(0x7ff8000000000000ll), prev_yz, prev_xi, sm0, f0);
+        const double x0 = ev ? P.nu[0] * beta : __longlong_as_double(0x7ff8000000000000ll);
+        if constexpr (TAB) planck_edge_t(x0, s_rows, prev_yz, prev_xi, sm0, f0);
+        else planck_edge0(x0, prev_yz, prev_xi, sm0, f0);
         prev_small = sm0;
         if (COUNT && sub == 0) eflops += f0;
       }
@@ -408,8 +416,11 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
         double hi_yz, hi_xi;
         bool hi_small;
         int hf;
-        planck_edge_w(evg ? t_nu * beta : __longlong_as_double(0x7ff8000000000000ll),
-                      (i & 1) * P.zero, hi_yz, hi_xi, hi_small, hf);
+{
+          const double xe = evg ? t_nu * beta : __longlong_as_double(0x7ff8000000000000ll);
+          if constexpr (TAB) planck_edge_t(xe, s_rows, hi_yz, hi_xi, hi_small, hf);
+          else planck_edge_w(xe, (i & 1) * P.zero, hi_yz, hi_xi, hi_small, hf);
+        }
         if (COUNT) eflops += hf;
         double lo_yz, lo_xi;
         bool lo_small;
@@ -738,18 +749,24 @@ __global__ void conserved_totals_kernel(const __grid_constant__ StatePtrs S, int
   }
 }
 
-// Diagnostic: the edge functions (the very planck_edge_w the update kernel uses) on an array of x;
-// tests pin them against the oracle's.  Whole warps run the loop so the warp-converged branches
-// see all 32 lanes; lanes past the end pass NaN (no branch) and store nothing.
+// Diagnostic: the edge functions the update kernels use, on an array of x; tests pin them against the oracle's.
+// form 0: planck_edge_t (per-interval rows; the instantiations for Nq <= 32 and the general kernel), form 1:
+// planck_edge_w (three branches; the Nq <= 64 instantiation).  Whole warps run the loop so the warp-converged
+// branches see all 32 lanes; lanes past the end pass NaN (no edge) and store nothing.
 __global__ void planck_edge_kernel(const double* __restrict__ x, long long n, double* __restrict__ yz,
-                                   double* __restrict__ xi, int* __restrict__ is_y, int zero) {
+                                   double* __restrict__ xi, int* __restrict__ is_y, int form, int zero) {
+  __shared__ __align__(16) double s_rows[kRows * kRowStride];
+  for (int t = threadIdx.x; t < kRows * kRowStride; t += blockDim.x) s_rows[t] = mgrhd_g_rows[t];
+  __syncthreads();
   const long long nround = (n + 31) / 32 * 32;
   for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < nround;
        i += (long long)gridDim.x * blockDim.x) {
     double a, b;
     bool small;
     int fl;
-    planck_edge_w(i < n ? x[i] : __longlong_as_double(0x7ff8000000000000ll), (int)(i & 1) * zero, a, b, small, fl);
+    const double xv = i < n ? x[i] : __longlong_as_double(0x7ff8000000000000ll);
+    if (form == 0) planck_edge_t(xv, s_rows, a, b, small, fl);
+    else planck_edge_w(xv, (int)(i & 1) * zero, a, b, small, fl);
     if (i < n) {
       MGRHD_CHK(i >= 0);
       yz[i] = a;

@@ -38,6 +38,9 @@ constexpr int kFlopEdgeSmall = 59;    // x < kXS: x, x^2, two 12-term Horner cha
 constexpr int kFlopEdgeMid = 95;      // kXS <= x < kXL: x, t, two degree-23 Horner chains
 constexpr int kFlopEdgeLarge = 96;    // x >= kXL: x, exp, 7 terms of (3+1) FMA, Xi with one reciprocal
 constexpr int kFlopEdgeZero = 32;     // x, exp that underflowed
+constexpr int kFlopRowSmall = 43;     // planck_edge_t, x < 1: x (1), t (2), two degree-9 Horner chains (36), x^3 (2), x^3 p (2)
+constexpr int kFlopRowMid = 39;       // planck_edge_t, 1 <= x < 8: x (1), t (2), two chains (36)
+constexpr int kFlopRowLarge = 71;     // planck_edge_t, x >= 8: x (1), t (2), two chains (36), exp (30), e^-x p (2)
 constexpr int kFlopGroupEval = 39;    // a2-a5 for one group at one trial T
 constexpr int kFlopCellEval = 27;     // T, a_R T^4, beta, scales, v, F_G, Eq. 49, sums over the cell's lanes
 constexpr int kFlopStepCell = 10;     // dx0, T > 0 check, E_gas update
@@ -129,5 +132,16 @@ struct alignas(16) PlanckTables {
   Pair l10[kLargeTerms];      // { 6C/n^3, 6C/n^4 }
   double mid_s, mid_o;
 };
+
+// Per-interval polynomial rows of the edge functions (mgrhd_planck.cuh, planck_edge_t): row 0 is x in [0, 0.5), rows
+// 1..56 the eight equal sub-intervals of each binade from [0.5, 1) to [32, 64) (the row index is read off the top bits
+// of x), row 57 is x >= 64.  A row is kRowTerms + 1 pairs: {centre, 2/width}, then {a_k, b_k} for k = 0..kRowTerms-1:
+//   x < 1:       Y  = x^3 sum a_k t^k,     Xi = x^3 sum b_k t^k      (15/pi^4 folded in)
+//   1 <= x < 8:  Z  = sum a_k t^k,         Xi = sum b_k t^k
+//   x >= 8:      Z  = e^-x sum a_k t^k,    Xi = e^-x sum b_k t^k,     t = (x - centre) 2/width  (row 57: t = x)
+constexpr int kRows = 58;
+constexpr int kRowTerms = 10;                      // degree 9: fit error below 1 ulp on every row
+constexpr int kRowStride = 2 * (kRowTerms + 1);    // doubles; 176 B puts eight neighbouring rows on distinct banks
+constexpr int kRowKey0 = 1022 * 8;                 // (high word >> 17) of 0.5
 
 }  // namespace mgrhd

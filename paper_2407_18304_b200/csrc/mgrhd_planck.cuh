@@ -4,9 +4,20 @@
 //   Y(x)  = (15/pi^4) int_0^x t^3/(e^t-1) dt,   Z(x) = 1 - Y(x),
 //   Xi(x) = (15/pi^4) x^4/(e^x-1)               (4 pi nu B_nu / c = a_R T^4 Xi(x)).
 //
-// Each edge returns ONE of Y (x < kXS) or Z (x >= kXS), so that a group difference never
+// Each edge returns ONE of Y (small x) or Z (large x), so that a group difference never
 // cancels in the Wien tail:  both Y: Y+ - Y-;  both Z: Z- - Z+;  straddling: 1 - Y- - Z+.
-// Three branches of BOUNDED cost:
+//
+// Two evaluations:
+//  * planck_edge_t -- per-interval polynomial ROWS (58 intervals: [0, 0.5), eight per binade up to 64, x >= 64),
+//    two degree-9 Horner chains whose coefficients each lane reads from its own row in shared memory:
+//    ONE code path whatever the lanes' x (only e^-x for x >= 8 is a warp-wide branch).  Y below x = 1.
+//    Used wherever the 10.2 KB of rows fit beside the kernel's state: Nq <= 32 and the general kernel.
+//    Measured against the three-branch form at config 4: -12 % warp instructions, -3 % time, 7 KB less code.
+//  * planck_edge_w -- three warp-wide branches with uniform-register coefficients (below), Y below x = kXS;
+//    kept for the Nq <= 64 instantiation, whose group state fills shared memory (rows read from global
+//    memory instead were 15 % slower).
+//
+// planck_edge_w: three branches of BOUNDED cost:
 //   x <  kXS        Maclaurin series in x^2, 12 even terms (truncation < 1e-19 relative);
 //   kXS <= x < kXL  degree-23 polynomial fits of Z and Xi (Chebyshev interpolants generated
 //                   in long double at init, abs. error < 1e-17 on functions of size 0.2-0.9);
@@ -21,6 +32,7 @@
 // planck_edge_w for why the second copy exists).
 extern "C" {
 __constant__ mgrhd::PlanckTables mgrhd_c_planck[2];
+__device__ double mgrhd_g_rows[mgrhd::kRows * mgrhd::kRowStride];   // per-interval rows, copied to shared memory by the kernels
 }
 
 namespace mgrhd {
@@ -105,6 +117,41 @@ __device__ __forceinline__ void planck_edge_w(double x, int which, double& yz, d
       flops = live ? kFlopEdgeLarge : kFlopEdgeZero;
     }
   }
+}
+
+// One-branch edge functions: every lane reads the polynomial row of the interval its x falls in (16-byte pairs from
+// shared memory, `rows` = a copy of mgrhd_g_rows) and runs two degree-9 Horner chains; only e^-x for x >= 8 is a
+// warp-wide branch.  Same contract as planck_edge_w except that Y is returned below x = 1 (not kXS), Z from there
+// on; NaN: no edge, (0, 0, large).  Accuracy: fit error < 1 ulp per row; Y = x^3 p(t) and Z = e^-x p(t) keep the
+// relative accuracy in both tails.
+__device__ __forceinline__ void planck_edge_t(double x, const double* rows, double& yz, double& xi, bool& small,
+                                              int& flops) {
+  const bool valid = x == x;
+  const double xs = valid ? x : 2.0;
+  int row = (__double2hiint(xs) >> 17) - (kRowKey0 - 1);
+  row = row < 0 ? 0 : (row > kRows - 1 ? kRows - 1 : row);
+  const double2* const r = reinterpret_cast<const double2*>(rows + row * kRowStride);
+  const bool inY = xs < 1.0, inE = xs >= 8.0;
+  double u = 1.0;
+  if (__any_sync(0xffffffffu, inE)) u = exp(-xs);          // 0 on underflow and for x = +inf
+  const bool live = !inE || u > 0.0;
+  const double xx = live ? xs : 1.0;                        // keeps inf * 0 out of the polynomials
+  const double2 cs = r[0];
+  const double t = (xx - cs.x) * cs.y;
+  double2 cf = r[kRowTerms];
+  double sy = cf.x, sx = cf.y;
+#pragma unroll
+  for (int k = kRowTerms - 1; k >= 1; --k) {
+    cf = r[k];
+    sy = fma(sy, t, cf.x);
+    sx = fma(sx, t, cf.y);
+  }
+  const double pref = inY ? xx * xx * xx : (inE ? u : 1.0);
+  const bool keep = valid && live;
+  yz = keep ? sy * pref : 0.0;
+  xi = keep ? sx * pref : 0.0;
+  small = valid && inY;
+  flops = !valid ? 0 : (inY ? kFlopRowSmall : (!inE ? kFlopRowMid : (live ? kFlopRowLarge : kFlopEdgeZero)));
 }
 
 // The same for callers outside a step loop (table copy 0), compiled once and called: keeps a second

@@ -65,20 +65,24 @@ def test_workload_parity(gpu, oracle_lib, index):
     assert abs(gs["outer_trips_total"] - os_["outer_trips_total"]) <= 0.02 * os_["outer_trips_total"]
 
 
-def test_planck_edge_functions_vs_oracle(gpu, oracle_lib):
-    """The kernel's three-branch edge functions against the oracle's long-double series, over every
-    branch, both sides of each switch point, the Wien tail down to underflow, and the 0 / inf edges."""
+@pytest.mark.parametrize("form", [0, 1])
+def test_planck_edge_functions_vs_oracle(gpu, oracle_lib, form):
+    """The kernel's edge functions (form 0: per-interval polynomial rows; form 1: three branches) against the oracle's
+    long-double series, over every row and branch, both sides of every switch point (each row boundary of form 0),
+    the Wien tail down to underflow, and the 0 / inf edges."""
     import torch
 
-    xs = np.concatenate([np.logspace(-6, np.log10(744.0), 4000), [0.0, 1.25, 5.5, np.nextafter(1.25, 0),
-                         np.nextafter(5.5, 0), 700.0, 745.0, 760.0, np.inf]])
-    yz, xi, is_y = (t.cpu().numpy() for t in gpu.planck_edge_functions(torch.from_numpy(xs).cuda()))
+    switch = 1.0 if form == 0 else 1.25
+    bounds = [0.5 * 2.0 ** b * (1 + m / 8) for b in range(7) for m in range(8)] + [64.0, 1.25, 5.5, 8.0]
+    xs = np.concatenate([np.logspace(-6, np.log10(744.0), 6000), [0.0, 700.0, 745.0, 760.0, np.inf],
+                         bounds, [np.nextafter(v, 0) for v in bounds], [np.nextafter(v, np.inf) for v in bounds]])
+    yz, xi, is_y = (t.cpu().numpy() for t in gpu.planck_edge_functions(torch.from_numpy(xs).cuda(), form))
     for x, a, b, k in zip(xs, yz, xi, is_y):
         ref = oracle_lib.planck_Y(x) if k else oracle_lib.planck_Z(x)
         rxi = oracle_lib.planck_Xi(x)
         assert abs(a - ref) <= 4e-15 * abs(ref) + 1e-290, (x, a, ref, k)
         assert abs(b - rxi) <= 4e-15 * abs(rxi) + 1e-290, (x, b, rxi)
-        assert k == (1 if x < 1.25 else 0)
+        assert k == (1 if x < switch else 0)
 
 
 def test_successive_calls_config5(gpu, oracle_lib):
