@@ -89,3 +89,46 @@ def conservation_residual(st0, st1, c, c_hat):
     with np.errstate(invalid="ignore", divide="ignore"):
         rP = float(np.max(np.where(Ps > 0, dP / Ps, dP)))
     return rE, rP
+
+
+def bad_cells(ref, got, st0, c, c_hat, afloor=AFLOOR):
+    """Indices of the cells with at least one entry outside the tolerance of compare()."""
+    Etot, Ps = scales(st0, c, c_hat)
+    n = Etot.shape[0]
+    bad = np.zeros(n, dtype=bool)
+    for key, S in (("Egas", Etot), ("Erad", Etot[None, :]), ("Frad", (c * Etot)[None, None, :]), ("mom", Ps[None, :])):
+        d = np.abs(got[key] - ref[key])
+        b = ~(d <= RTOL * np.abs(ref[key]) + afloor * S)
+        bad |= b.reshape(-1, n).any(axis=0)
+    return np.nonzero(bad)[0]
+
+
+def unexplained_cells(oracle, wl, st0, got, dt, cells, afloor=AFLOOR, factors=(2.0, 0.5, 4.0, 0.25)):
+    """The stopping tests (Eq. 49, reading S10) are floating-point comparisons that decide an
+    INTEGER, the number of evaluations and outer trips; a cell whose residual sits within rounding of a threshold may
+    stop one trip earlier in one implementation than in the other, and the two results, both accepted by the paper's
+    rule, then differ by one (small) step instead of by rounding.  Such a cell is recognised here by what is unique
+    about it: the GPU's result must equal, to the standing tolerance, the ORACLE's own result with the three
+    thresholds (newton_tol, outer_tol, outer_rel_tol) moved by a factor of 2 or 4 either way -- i.e. the oracle one
+    decision earlier or later.  Returns the cells of `cells` for which no such run matches: those are arithmetic
+    differences and stay failures.  (used by bench.py's parity sample, which checks 1e5-3e5
+    cells per run; the pytest parity cases compare strictly.)"""
+    import copy
+
+    cells = np.asarray(cells, dtype=np.int64)
+    left = cells
+    sub = lambda st, idx: {k: (None if v is None else np.ascontiguousarray(v[..., idx])) for k, v in st.items()}
+    for f in factors:
+        if left.size == 0:
+            break
+        w2 = copy.copy(wl)
+        w2.newton_tol, w2.outer_tol, w2.outer_rel_tol = wl.newton_tol * f, wl.outer_tol * f, wl.outer_rel_tol * f
+        s0 = sub(st0, left)
+        ref = {k: (None if v is None else v.copy()) for k, v in s0.items()}
+        oracle.source_update(oracle_model(oracle, w2), ref, dt, wl.c, wl.c_hat)
+        scale = dict(s0)
+        if s0.get("Srad") is not None:
+            scale["Erad"] = s0["Erad"] + s0["Srad"]
+        still = bad_cells(ref, sub(got, left), scale, wl.c, wl.c_hat, afloor=afloor)
+        left = left[still]
+    return left

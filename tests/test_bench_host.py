@@ -55,3 +55,31 @@ def test_gpus_flag_must_match_world_size():
     r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--cells", "64"], env=env,
                        capture_output=True, text=True, timeout=300)
     assert r.returncode != 0 and "WORLD_SIZE" in (r.stderr + r.stdout)
+
+
+def test_stopping_decisions_are_told_apart_from_arithmetic_differences():
+    """parity_util.unexplained_cells (used by bench.py's parity sample): a result that is the oracle's own with the
+    stopping thresholds moved is 'a stopping test on the other side of its threshold'; a perturbed result is not."""
+    import copy
+
+    import oracle
+    from parity_util import bad_cells, oracle_model, unexplained_cells
+
+    oracle.build()
+    wl = W.workload(2, ncells=400)
+    st0 = W.to_numpy(wl.make_state())
+    ref = {k: (None if v is None else v.copy()) for k, v in st0.items()}
+    oracle.source_update(oracle_model(oracle, wl), ref, wl.dt, wl.c, wl.c_hat)
+    loose = copy.copy(wl)
+    loose.newton_tol, loose.outer_tol, loose.outer_rel_tol = 2 * wl.newton_tol, 2 * wl.outer_tol, 2 * wl.outer_rel_tol
+    got = {k: (None if v is None else v.copy()) for k, v in st0.items()}
+    oracle.source_update(oracle_model(oracle, loose), got, wl.dt, wl.c, wl.c_hat)    # stops earlier in some cells
+    assert bad_cells(ref, ref, st0, wl.c, wl.c_hat).size == 0
+    early = bad_cells(ref, got, st0, wl.c, wl.c_hat, afloor=1e-17)                     # (tight floor: make some cells differ)
+    assert early.size > 0
+    assert unexplained_cells(oracle, wl, st0, got, wl.dt, early, afloor=1e-17).size == 0
+    got["Erad"][3, 7] *= 1.0 + 1e-8                                                   # an arithmetic error
+    got["mom"][1, 11] += 1e-7 * abs(got["mom"][1, 11]) + 1e-12
+    cells = bad_cells(ref, got, st0, wl.c, wl.c_hat)
+    assert set(cells) >= {7, 11}
+    assert set(unexplained_cells(oracle, wl, st0, got, wl.dt, cells)) == {7, 11}
