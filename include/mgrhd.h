@@ -198,9 +198,9 @@ long long mgrhd_launch_count(const mgrhd_ctx *ctx);
  * call outside a graph capture.
  * Limits.  Only the models the tuned kernel runs: spectrum 0, opacity_kind 0 or 1, outer_mode 0 (anything else:
  * MGRHD_ERR_ARG).  The scratch a launch needs is 256 + 24 NQL threads_per_CTA CTAs bytes (NQL = 4, 8, 8, 8, 16 and
- * 256, 384, 384, 384, 288 threads for Nq <= 4, 8, 16, 32, 64; CTAs = min(resident CTAs of the device,
+ * 256, 384, 384, 384, 256 threads for Nq <= 4, 8, 16, 32, 64; CTAs = min(resident CTAs of the device,
  * ceil(ncells / cells per CTA))): on a 148-SM B200 every Nq <= 32 fits at any ncells (10.9 MB); 32 < Nq <= 64 fits
- * up to 8136 cells.  A launch that needs more returns MGRHD_ERR_SIZE (mgrhd_last_error() states both numbers)
+ * up to 8192 cells.  A launch that needs more returns MGRHD_ERR_SIZE (mgrhd_last_error() states both numbers)
  * and does nothing.
  * Sharing.  Every call on a device uses the same arrays, which keep the previous call's contents: the call clears
  * the work counter and the counters itself (stream-ordered memsets), the rest of the scratch is written before it is
@@ -217,9 +217,9 @@ int mgrhd_source_update_static(const double *edges, int Nq, const mgrhd_units *u
 /* Diagnostic: the kernels' Planck edge functions on n DEVICE values x >= 0 (x = h nu/(k_B T)):
  *   is_y[i] = 1: yz[i] = Y(x) = (15/pi^4) int_0^x t^3/(e^t-1) dt;  is_y[i] = 0: yz[i] = 1 - Y(x);
  *   xi[i] = (15/pi^4) x^4/(e^x-1).  (Eq. 11 applied to B_nu.)
- * form 0: the per-interval polynomial rows (Y below x = 1) the update uses for Nq <= 32 and in the general kernel
- * (free-slope spectrum, opacity_kind 2, outer_mode 1); form 1: the three-branch evaluation (Y below x = 1.25) it
- * uses for 32 < Nq <= 64.  Other values: MGRHD_ERR_ARG.
+ * form 0: the per-interval polynomial rows (Y below x = 1) every update kernel uses; form 1: the three-branch
+ * evaluation (Y below x = 1.25) kept for a kernel instantiation without room for the rows (none is dispatched
+ * today).  Other values: MGRHD_ERR_ARG.
  * Stream-ordered. */
 int mgrhd_planck_edge_functions(const double *x_dev, long long n, double *yz_dev, double *xi_dev,
                                 int *is_y_dev, int form, void *cuda_stream);

@@ -256,7 +256,7 @@ struct Inst {
     else if ((Nq) <= 8) { WHAT(1, 8, 384); }                   \
     else if ((Nq) <= 16) { WHAT(2, 8, 384); }                  \
     else if ((Nq) <= 32) { WHAT(4, 8, 384); }                  \
-    else { WHAT(4, 16, 288); }                                 \
+    else { WHAT(4, 16, 256); }                                 \
   } while (0)
 
 // Fills ctx->cfg_* for ctx->P.Nq (called once by mgrhd_init).

@@ -183,7 +183,9 @@ source_update_kernel(const __grid_constant__ Params P, const __grid_constant__ S
   constexpr int TS = 10;   // row stride in doubles: 80 B puts the L rows of a step on distinct banks
   __shared__ __align__(16) double s_tab[(kMaxG + 1) * TS];
   // Per-interval rows of the edge functions (planck_edge_t) where the instantiation leaves room for them beside its
-  // group state; the Nq <= 64 instantiation fills shared memory and keeps the three-branch planck_edge_w.
+  // group state: every instantiation mgrhd_api.cu dispatches to (Nq <= 64 runs 256 threads for that reason: eight
+  // warps with the rows beat nine with the three-branch planck_edge_w); the three-branch form
+  // remains for an instantiation whose state fills shared memory.
   constexpr bool TAB = (size_t)SL_COUNT * NQL * THREADS * sizeof(double) + 6144 + kRows * kRowStride * sizeof(double) <= 227 * 1024;
   __shared__ __align__(16) double s_rows[TAB ? kRows * kRowStride : 2];
   if constexpr (TAB)
@@ -771,7 +773,7 @@ __global__ void conserved_totals_kernel(const __grid_constant__ StatePtrs S, int
 
 // Diagnostic: the edge functions the update kernels use, on an array of x; tests pin them against the oracle's.
 // form 0: planck_edge_t (per-interval rows; the instantiations for Nq <= 32 and the general kernel), form 1:
-// planck_edge_w (three branches; the Nq <= 64 instantiation).  Whole warps run the loop so the warp-converged
+// planck_edge_w (three branches; an instantiation without room for the rows -- none of the dispatched ones).  Whole warps run the loop so the warp-converged
 // branches see all 32 lanes; lanes past the end pass NaN (no edge) and store nothing.
 __global__ void planck_edge_kernel(const double* __restrict__ x, long long n, double* __restrict__ yz,
                                    double* __restrict__ xi, int* __restrict__ is_y, int form, int zero) {

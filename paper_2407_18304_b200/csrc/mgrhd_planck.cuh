@@ -11,11 +11,12 @@
 //  * planck_edge_t -- per-interval polynomial ROWS (58 intervals: [0, 0.5), eight per binade up to 64, x >= 64),
 //    two degree-9 Horner chains whose coefficients each lane reads from its own row in shared memory:
 //    ONE code path whatever the lanes' x (only e^-x for x >= 8 is a warp-wide branch).  Y below x = 1.
-//    Used wherever the 10.2 KB of rows fit beside the kernel's state: Nq <= 32 and the general kernel.
-//    Measured against the three-branch form at config 4: -12 % warp instructions, -3 % time, 7 KB less code.
+//    Used wherever the 10.2 KB of rows fit beside the kernel's state: every dispatched instantiation of the tuned
+//    kernel and the general kernel.  Measured against the three-branch form at config 4: -12 % warp instructions,
+//    -3 % time, 7 KB less code; at Nq = 64, where the rows cost a ninth warp, -4 %.
 //  * planck_edge_w -- three warp-wide branches with uniform-register coefficients (below), Y below x = kXS;
-//    kept for the Nq <= 64 instantiation, whose group state fills shared memory (rows read from global
-//    memory instead were 15 % slower).
+//    for an instantiation whose group state fills shared memory (rows read from global memory instead were
+//    15 % slower) and as the second form of the diagnostic entry point.
 //
 // planck_edge_w: three branches of BOUNDED cost:
 //   x <  kXS        Maclaurin series in x^2, 12 even terms (truncation < 1e-19 relative);

@@ -103,9 +103,9 @@ def test_static_entry_point_allocates_nothing_and_states_its_limit(gpu):
     torch.cuda.synchronize()
     free1, _ = torch.cuda.mem_get_info()
     assert free1 == free0, (free0, free1)
-    # Nq = 64: 256 + 24 * 16 * 288 bytes of scratch per CTA, one CTA per 72 cells up to one per SM
+    # Nq = 64: 256 + 24 * 16 * 256 bytes of scratch per CTA, one CTA per 64 cells up to one per SM
     sms = torch.cuda.get_device_properties(0).multi_processor_count
-    per_cta = 24 * 16 * 288
+    per_cta = 24 * 16 * 256
     big = W.workload(5, ncells=72 * 400)
     bdev = to_dev(W.to_numpy(big.make_state()))
     keep = W.to_numpy(bdev)
@@ -116,7 +116,7 @@ def test_static_entry_point_allocates_nothing_and_states_its_limit(gpu):
         now = W.to_numpy(bdev)
         for k in FIELDS:
             assert np.array_equal(keep[k], now[k]), k                     # rejected: nothing was touched
-    small = W.workload(5, ncells=72 * 100 + 5)                            # 101 CTAs: 11.2 MB, fits
+    small = W.workload(5, ncells=72 * 100 + 5)                            # 113 CTAs: 11.1 MB, fits
     st0 = W.to_numpy(small.make_state())
     refs, rstats = existing_path(gpu, small, st0, [small.dt])
     sdev = to_dev(st0)
